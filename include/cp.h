@@ -1,0 +1,220 @@
+/*
+ * cp.h -- C ABI of libcp: the mixed-batch paged-attention step of a chunked-prefill
+ * serving iteration on one NVIDIA B200 (sm_100a), plus the host-side scheduler that
+ * forms each iteration (aging / LPRS / APC of arxiv/paper_2606_09061).
+ *
+ * Plain C, plain pointers, no torch types.  Every pointer argument says whether it is
+ * HOST or DEVICE memory.  All functions return int: CP_OK (0) or a negative error;
+ * nothing throws or aborts; cp_last_error() gives a thread-local message.
+ *
+ * Ownership: the caller owns every device tensor it passes (q, k_new, v_new, kv_cache,
+ * out) and the CUDA stream.  The library owns its context, device metadata, the
+ * split-KV partial workspace, pinned staging and CUDA events, all allocated in
+ * cp_create from the limits in cp_config; nothing is allocated and nothing
+ * synchronises afterwards, except cp_latency_table (may wait on the newest timed
+ * step) and cp_destroy.
+ *
+ * The operation (PAPER.md:61, :87 chunked-prefill mixed batch; PAPER.md:41 paged KV;
+ * defined in DESIGN.md section 2, restating SURVEY.md 8(c1)): for request j, row
+ * i < q_len_j, q head h, g = h / (Hq/Hkv), over keys t in [0, ctx_off_j + i]:
+ *     s_t = sm_scale * <q[tok(j,i),h,:], K_j[t,g,:]>,  out = softmax_t(s) . V_j[:,g,:]
+ * where K_j[t], V_j[t] live in page block_table_j[t / B], slot t % B.  A decode is
+ * simply q_len == 1.  Stale data in page tails / other pages never influences the
+ * result (finite stale values; see DESIGN.md for NaN tails).
+ */
+#ifndef CP_H_
+#define CP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CP_OK          0
+#define CP_EINVAL     (-1)   /* bad argument / shape / table too short            */
+#define CP_ECAPACITY  (-2)   /* exceeds a limit fixed at cp_create               */
+#define CP_ECUDA      (-3)   /* a CUDA call failed (message in cp_last_error)     */
+#define CP_ESTATE     (-4)   /* wrong call order (e.g. step before build_batch)   */
+
+#define CP_NUM_RAW_FEATURES 11   /* Table 1 */
+#define CP_NUM_FEATURES     16   /* + Table 2 */
+
+typedef struct cp_ctx cp_ctx;       /* opaque */
+typedef struct cp_sched cp_sched;   /* opaque */
+
+/* ---------------------------------------------------------------------------------
+ * KV cache layout (part of the ABI), bf16, one pool per layer, layer-major:
+ *     kv_cache[layer][block][kv: 0 = K, 1 = V][kv_head][slot in 0..B-1][d in 0..D-1]
+ * A (block, kv, head) slab is B*D*2 bytes contiguous (4 KiB at B 16, D 128); K and V
+ * of a block are adjacent.  cp_attention_step takes the pointer to the LAYER's pool.
+ * ------------------------------------------------------------------------------- */
+typedef struct {
+    int32_t num_q_heads;      /* Hq                                               */
+    int32_t num_kv_heads;     /* Hkv, divides Hq; G = Hq/Hkv in {1,2,4,8,16}      */
+    int32_t head_dim;         /* D in {64, 128}                                   */
+    int32_t block_size;       /* B, tokens per page: 16                           */
+    int32_t num_layers;       /* only used to size the latency ring; >= 1         */
+    int64_t num_blocks;       /* pages per layer pool                             */
+    float   sm_scale;         /* e.g. 1/sqrt(D), applied in fp32                  */
+    int32_t max_tokens;       /* limit on T = sum q_len per batch                 */
+    int32_t max_reqs;         /* limit on requests per batch                      */
+    int64_t max_total_pages;  /* limit on sum of n_blocks over the batch          */
+    int64_t max_partial_rows; /* split-KV workspace rows ((D+2) fp32 each);
+                                 0 = default 4 * max_tokens * Hq                  */
+    int32_t device;           /* CUDA device ordinal                              */
+    int32_t kernel_variant;   /* 0 = default (tensor-core path where built),
+                                 1 = force the SIMT reference kernels (debug)     */
+} cp_config;
+
+/* One request of the iteration.  HOST pointers. */
+typedef struct {
+    int64_t        req_id;
+    int32_t        q_len;        /* >= 1 tokens scheduled this iteration          */
+    int32_t        ctx_off;      /* >= 0 tokens already in the cache before them  */
+    const int32_t* block_table;  /* HOST: n_blocks page ids in [0, num_blocks)    */
+    int32_t        n_blocks;     /* n_blocks * B >= ctx_off + q_len               */
+} cp_req_desc;
+
+/* One timed step: the 11 raw features of Table 1 + measured us
+ * ("ground-truth batch latency measured by a high-resolution timer"). */
+typedef struct {
+    float   feat[CP_NUM_RAW_FEATURES]; /* prefill_tokens, decode_tokens,
+          batch_request_count, sum_decode_context_len, max_decode_context_len,
+          prefill_processed_tokens, max_prefill_processed_tokens, gpu_mem_used_mb,
+          gpu_mem_free_mb, cuda_allocated_mb, cuda_reserved_mb                    */
+    float   us;                 /* device time of cp_attention_step (CUDA events)  */
+    int32_t n_prefill;          /* requests with q_len > 1                         */
+    int32_t n_decode;           /* requests with q_len == 1                        */
+    int32_t layer;
+    int64_t iter;               /* index of the cp_build_batch this step ran under */
+} cp_latency_row;
+
+const char* cp_last_error(void);
+
+/* Create / destroy a context.  cfg: HOST.  Allocates everything the context will ever
+ * need.  Errors: CP_EINVAL (unsupported shape), CP_ECUDA. */
+int cp_create(const cp_config* cfg, cp_ctx** out);
+int cp_destroy(cp_ctx* ctx);
+
+/* H1: pack the iteration's request descriptors into device metadata
+ * (cu_q, q_len, ctx_off, flat block table, work list, combine list) with ONE async
+ * host->device copy on `cuda_stream` (a cudaStream_t, may be NULL = default stream).
+ * reqs: HOST array of n_reqs descriptors, any mix/order of prefill chunks and decodes;
+ * token order of q/out = descriptor order, rows of a request contiguous.
+ * A page id may appear in only one request of the batch.  The metadata stays valid for
+ * any number of cp_attention_step calls (all layers) until the next cp_build_batch.
+ * Errors: CP_EINVAL (q_len < 1, ctx_off < 0, table too short, page id out of range),
+ * CP_ECAPACITY (limits of cp_config), CP_ECUDA.  On error the previous batch is kept. */
+int cp_build_batch(cp_ctx* ctx, const cp_req_desc* reqs, int32_t n_reqs,
+                   void* cuda_stream);
+
+/* H2-H6: run the attention step of one layer for the current batch, asynchronously on
+ * `cuda_stream`, bracketed by a CUDA-event pair that cp_latency_table later resolves.
+ *   q        DEVICE [T, Hq, D]  bf16
+ *   k_new    DEVICE [T, Hkv, D] bf16, or NULL = caller already wrote the pages
+ *   v_new    DEVICE [T, Hkv, D] bf16 (NULL iff k_new is NULL)
+ *   kv_cache DEVICE the layer's pool [num_blocks][2][Hkv][B][D] bf16; the new rows are
+ *            appended in place before anything attends (H2)
+ *   out      DEVICE [T, Hq, D]  bf16, every row written
+ * All pointers 16-byte aligned.  Errors: CP_ESTATE (no batch built), CP_EINVAL, CP_ECUDA. */
+int cp_attention_step(cp_ctx* ctx, int32_t layer, const void* q, const void* k_new,
+                      const void* v_new, void* kv_cache, void* out, void* cuda_stream);
+
+/* H6: drain the ring of timed steps, oldest first, into rows (HOST, capacity cap);
+ * *n_out receives the count.  Waits for the newest recorded step to finish.  The memory
+ * features are what cp_set_memory_stats last stored (zeros if never called). */
+int cp_latency_table(cp_ctx* ctx, cp_latency_row* rows, int32_t cap, int32_t* n_out);
+
+/* Table 1's four memory features come from the caller's allocator (PyTorch owns device
+ * memory here); values in MB, copied into subsequent latency rows. */
+int cp_set_memory_stats(cp_ctx* ctx, float gpu_mem_used_mb, float gpu_mem_free_mb,
+                        float cuda_allocated_mb, float cuda_reserved_mb);
+
+/* Introspection of the current batch (for tests and the roofline report). */
+typedef struct {
+    int32_t n_reqs, n_tokens, n_work_items, n_combine_items;
+    int32_t n_tc_items;          /* items routed to the tensor-core tile path      */
+    int64_t n_partial_rows;      /* workspace rows in use                          */
+    int32_t kernels_per_step;    /* kernel launches one cp_attention_step issues   */
+    int32_t grid_attn, grid_combine;
+} cp_batch_info;
+int cp_get_batch_info(cp_ctx* ctx, cp_batch_info* info);
+
+/* ---------------------------------------------------------------------------------
+ * Host-side scheduler (no GPU).  H0 of SURVEY.md 8(a).  Forms one iteration under a
+ * token budget or a target time: decode first, prefills ranked by the
+ * aging key K_i = -alpha a_i + beta r_i (Eq. 4) in a max-heap
+ * (PAPER.md:101), chunk by Eq. 6-7 (token budget) or Algorithm 1 (LPRS, Eq. 8-11,
+ * PAPER.md:165-253), gated by APC (Eq. 12-14).  Readings of silent
+ * points: DESIGN.md S1-S14.  Output is bit-identical to oracle/ref_scheduler.py.
+ * ------------------------------------------------------------------------------- */
+#define CP_MODE_TOKEN_BUDGET 0
+#define CP_MODE_LPRS         1
+#define CP_PRED_LINEAR       0    /* T_hat = sum_k w[k] z[k], k ascending             */
+#define CP_PRED_MLP          1    /* 16->128->64->32->1 ReLU (Table 7)  */
+
+typedef struct {
+    double  alpha;          /* > 0, per second of waiting (Eq. 1)                     */
+    double  beta;           /* < 0, per remaining prefill token (Eq. 1)               */
+    int32_t B_max;          /* hard token budget per round (Eq. 6)                    */
+    int32_t S_max;          /* maximum sequences per batch (Eq. 12)                   */
+    int32_t mode;           /* CP_MODE_*                                              */
+    int32_t apc;            /* 0/1: Active Prefill Control                            */
+    int32_t Delta;          /* search granularity (Eq. 8)                             */
+    int32_t C_max;          /* configured max active prefills (Eq. 12)                */
+    int32_t L_min;          /* minimum effective chunk (Eq. 12-13)                    */
+    int32_t block_size;     /* tokens per page                                        */
+    int64_t num_blocks;     /* pages in the pool                                      */
+    double  T_star;         /* target latency budget, same unit as the predictor      */
+    double  lambda_u;       /* underfill penalty (Eq. 10)                             */
+    double  lambda_o;       /* overflow penalty, > lambda_u (Eq. 10)                  */
+    double  page_mb;        /* MB per page, for the deterministic memory features     */
+    int32_t pred_kind;      /* CP_PRED_*                                              */
+    int32_t n_pred_weights; /* 16 (linear) or 12673 (MLP)                             */
+    const double* pred_weights;   /* HOST, copied                                     */
+    const double* feat_mu;        /* HOST [16] or NULL (= 0): z = (x - mu) * inv_sigma */
+    const double* feat_inv_sigma; /* HOST [16] or NULL (= 1)                          */
+} cp_sched_config;
+
+typedef struct {
+    int64_t n_iters;
+    int64_t blocked_by_activity_cap;   /* Table 10 */
+    int64_t blocked_by_min_chunk;      /* Table 10 */
+    int64_t used_pages;
+    int32_t n_waiting, n_decoding, n_future;
+} cp_sched_stats;
+
+int cp_sched_create(const cp_sched_config* cfg, cp_sched** out);
+int cp_sched_destroy(cp_sched* s);
+/* Register a request (arrival in integer microseconds).  CP_EINVAL: prompt_len < 1,
+ * output_len < 1 or duplicate id; CP_ECAPACITY: can never fit the pool. */
+int cp_sched_add_request(cp_sched* s, int64_t req_id, int64_t arrival_us,
+                         int32_t prompt_len, int32_t output_len);
+/* Form one iteration at clock now_us: decodes first in (arrival_us, req_id) order, then
+ * prefill chunks in selection order.  out: HOST array of capacity cap; each
+ * block_table pointer stays valid until the next cp_sched_commit / cp_sched_destroy.
+ * *n_out == 0 means nothing is runnable (no commit needed; advance the clock to
+ * cp_sched_next_arrival).  CP_ESTATE if the previous iteration was not committed,
+ * CP_ECAPACITY if cap is too small. */
+int cp_sched_next(cp_sched* s, int64_t now_us, cp_req_desc* out, int32_t cap,
+                  int32_t* n_out);
+/* Advance request states after the iteration ran for iter_us (Eq. 2, requeue, TTFT). */
+int cp_sched_commit(cp_sched* s, int64_t iter_us);
+int cp_sched_next_arrival(cp_sched* s, int64_t* arrival_us);  /* -1 if none */
+int cp_sched_has_work(cp_sched* s, int32_t* has_work);
+int cp_sched_get_stats(cp_sched* s, cp_sched_stats* st);
+/* Per-request result: TTFT and finish time in us (-1 if not reached yet). */
+int cp_sched_request_times(cp_sched* s, int64_t req_id, int64_t* ttft_us,
+                           int64_t* finish_us);
+/* Exposed for pinning against the reference (pure functions of the config): */
+int cp_sched_predict(cp_sched* s, const double* x16, double* t_hat);
+int cp_sched_select_chunk(cp_sched* s, int32_t r_i, int32_t ctx_i, int32_t U_t,
+                          int32_t n_dec, int64_t sum_ctx, int32_t max_ctx,
+                          int32_t pf_tokens, int32_t n_pf, int64_t pf_proc,
+                          int32_t pf_proc_max, int32_t* c_star);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CP_H_ */

@@ -1,0 +1,459 @@
+// cp_api.cu -- libcp's C ABI for the GPU path: context, batch packing (H1), the attention
+// step launcher (H2-H5) and the latency table (H6).  See include/cp.h for the contract.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "cp_internal.h"
+#include "cp_kernels_simt.cuh"
+#ifdef CP_WITH_TC
+#include "cp_kernels_tc.cuh"
+#endif
+
+using namespace cp;
+
+#define CP_CUDA(call)                                                                     \
+    do {                                                                                  \
+        cudaError_t e__ = (call);                                                         \
+        if (e__ != cudaSuccess) {                                                         \
+            cp_set_error("%s:%d %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
+            return CP_ECUDA;                                                              \
+        }                                                                                 \
+    } while (0)
+
+namespace {
+
+constexpr int kRing = 4096;           // timed steps kept for cp_latency_table
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct TimedStep {
+    cudaEvent_t start = nullptr, stop = nullptr;
+    cp_latency_row row{};
+};
+
+}  // namespace
+
+struct cp_ctx {
+    cp_config cfg{};
+    Shape shape{};
+    int n_sm = 148;
+    int tq = 32;                       // tokens per Q tile = 128 / G
+    bool use_tc = false;
+
+    // limits
+    size_t max_items = 0, max_combine = 0, meta_cap = 0;
+    int64_t max_partial_rows = 0;
+
+    // device
+    uint8_t* d_meta = nullptr;
+    float* d_part_o = nullptr;
+    float2* d_part_ml = nullptr;
+    int32_t* d_counter = nullptr;      // persistent-kernel work counter
+    // pinned staging, double buffered
+    uint8_t* h_stage[2] = {nullptr, nullptr};
+    cudaEvent_t stage_done[2] = {nullptr, nullptr};
+    bool stage_used[2] = {false, false};
+    int stage_idx = 0;
+
+    // current batch
+    bool have_batch = false;
+    BatchMeta meta{};
+    cp_batch_info info{};
+    int64_t iter = -1;
+    float feat[CP_NUM_RAW_FEATURES] = {0};
+    float mem_stats[4] = {0, 0, 0, 0};
+    int32_t n_prefill = 0, n_decode = 0;
+
+    // latency ring
+    std::vector<TimedStep> ring;
+    int64_t ring_head = 0, ring_tail = 0;   // [tail, head) are undrained
+
+    // host scratch reused across build_batch calls (no allocation in steady state)
+    std::vector<WorkItem> items, sorted;
+    std::vector<CombineItem> combines;
+    std::vector<int32_t> bucket;
+};
+
+extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
+    if (!cfg || !out) { cp_set_error("cp_create: null argument"); return CP_EINVAL; }
+    const int Hq = cfg->num_q_heads, Hkv = cfg->num_kv_heads, D = cfg->head_dim;
+    if (Hq < 1 || Hkv < 1 || Hq % Hkv != 0) { cp_set_error("cp_create: Hq must be a multiple of Hkv"); return CP_EINVAL; }
+    const int G = Hq / Hkv;
+    if (!(G == 1 || G == 2 || G == 4 || G == 8 || G == 16)) { cp_set_error("cp_create: G = Hq/Hkv must be in {1,2,4,8,16}"); return CP_EINVAL; }
+    if (!(D == 64 || D == 128)) { cp_set_error("cp_create: head_dim must be 64 or 128"); return CP_EINVAL; }
+    if (cfg->block_size != 16) { cp_set_error("cp_create: block_size must be 16"); return CP_EINVAL; }
+    if (cfg->num_blocks < 1 || cfg->max_tokens < 1 || cfg->max_reqs < 1 || cfg->max_total_pages < 1 ||
+        cfg->num_layers < 1) { cp_set_error("cp_create: limits must be positive"); return CP_EINVAL; }
+    if ((int64_t)cfg->num_blocks * 2 * Hkv >= (int64_t)1 << 31) { cp_set_error("cp_create: pool too large for 32-bit slab index"); return CP_EINVAL; }
+
+    CP_CUDA(cudaSetDevice(cfg->device));
+    cp_ctx* c = new cp_ctx();
+    c->cfg = *cfg;
+    c->shape = Shape{Hq, Hkv, D, cfg->block_size, G, cfg->sm_scale};
+    c->tq = 128 / G;
+    cudaDeviceProp prop{};
+    if (cudaGetDeviceProperties(&prop, cfg->device) == cudaSuccess) c->n_sm = prop.multiProcessorCount;
+#ifdef CP_WITH_TC
+    c->use_tc = (cfg->kernel_variant == 0) && prop.major == 10;
+#endif
+    if (cfg->kernel_variant == 0 && !c->use_tc) {
+        // the default variant is the tensor-core path; refuse to run it silently on
+        // something else (no fallback dispatch).  Variant 1 is the explicit SIMT path.
+#ifdef CP_WITH_TC
+        delete c;
+        cp_set_error("cp_create: kernel_variant 0 needs an sm_100 device");
+        return CP_EINVAL;
+#endif
+    }
+    const size_t q_tiles = (size_t)cfg->max_reqs + (size_t)cfg->max_tokens / c->tq + 1;
+    c->max_items = q_tiles * Hkv + (size_t)c->n_sm * 16 + 64;
+    c->max_combine = q_tiles * Hkv;
+    c->max_partial_rows = cfg->max_partial_rows > 0 ? cfg->max_partial_rows
+                                                     : (int64_t)4 * cfg->max_tokens * Hq;
+    size_t cap = 0;
+    cap += align_up(sizeof(int32_t) * (cfg->max_reqs + 1), 16) * 2;      // cu_q, bt_off
+    cap += align_up(sizeof(int32_t) * cfg->max_reqs, 16) * 2;            // q_len, ctx_off
+    cap += align_up(sizeof(int32_t) * (size_t)cfg->max_total_pages, 16);
+    cap += align_up(sizeof(int32_t) * (size_t)cfg->max_tokens, 16);      // tok_req
+    cap += align_up(sizeof(WorkItem) * c->max_items, 16);
+    cap += align_up(sizeof(CombineItem) * c->max_combine, 16);
+    c->meta_cap = cap;
+
+    cudaError_t e = cudaSuccess;
+    auto chk = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+    chk(cudaMalloc(&c->d_meta, cap));
+    chk(cudaMalloc(&c->d_part_o, sizeof(float) * (size_t)c->max_partial_rows * D));
+    chk(cudaMalloc(&c->d_part_ml, sizeof(float2) * (size_t)c->max_partial_rows));
+    chk(cudaMalloc(&c->d_counter, sizeof(int32_t) * 4));
+    chk(cudaMemset(c->d_counter, 0, sizeof(int32_t) * 4));
+    for (int i = 0; i < 2; ++i) {
+        chk(cudaMallocHost(&c->h_stage[i], cap));
+        chk(cudaEventCreateWithFlags(&c->stage_done[i], cudaEventDisableTiming));
+    }
+    c->ring.resize(kRing);
+    for (auto& t : c->ring) {
+        chk(cudaEventCreate(&t.start));
+        chk(cudaEventCreate(&t.stop));
+    }
+    if (e != cudaSuccess) {
+        cp_set_error("cp_create: CUDA allocation failed: %s", cudaGetErrorString(e));
+        cp_destroy(c);
+        return CP_ECUDA;
+    }
+    c->items.reserve(c->max_items);
+    c->sorted.reserve(c->max_items);
+    c->combines.reserve(c->max_combine);
+    *out = c;
+    return CP_OK;
+}
+
+extern "C" int cp_destroy(cp_ctx* c) {
+    if (!c) return CP_OK;
+    cudaSetDevice(c->cfg.device);
+    cudaDeviceSynchronize();
+    cudaFree(c->d_meta);
+    cudaFree(c->d_part_o);
+    cudaFree(c->d_part_ml);
+    cudaFree(c->d_counter);
+    for (int i = 0; i < 2; ++i) {
+        if (c->h_stage[i]) cudaFreeHost(c->h_stage[i]);
+        if (c->stage_done[i]) cudaEventDestroy(c->stage_done[i]);
+    }
+    for (auto& t : c->ring) {
+        if (t.start) cudaEventDestroy(t.start);
+        if (t.stop) cudaEventDestroy(t.stop);
+    }
+    delete c;
+    return CP_OK;
+}
+
+// ------------------------------------------------------------------------------------
+// H1: cp_build_batch -- validate, plan the work list, pack, one async H2D copy.
+// ------------------------------------------------------------------------------------
+extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs, void* stream_) {
+    if (!c || (!reqs && n_reqs > 0) || n_reqs < 0) { cp_set_error("cp_build_batch: bad argument"); return CP_EINVAL; }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const Shape& sh = c->shape;
+    const int B = sh.B, G = sh.G, TQ = c->tq;
+    if (n_reqs > c->cfg.max_reqs) { cp_set_error("cp_build_batch: %d requests > max_reqs %d", n_reqs, c->cfg.max_reqs); return CP_ECAPACITY; }
+
+    // ---- validate + totals ------------------------------------------------------------
+    int64_t T = 0, P = 0, total_tiles = 0;
+    float f_pf_tokens = 0, f_dec = 0, f_sum_ctx = 0, f_max_ctx = 0, f_pf_proc = 0, f_pf_proc_max = 0;
+    int32_t n_prefill = 0, n_decode = 0;
+    for (int j = 0; j < n_reqs; ++j) {
+        const cp_req_desc& r = reqs[j];
+        if (r.q_len < 1 || r.ctx_off < 0 || r.n_blocks < 0 || (!r.block_table && r.n_blocks > 0)) {
+            cp_set_error("cp_build_batch: request %d: q_len %d ctx_off %d n_blocks %d", j, r.q_len, r.ctx_off, r.n_blocks);
+            return CP_EINVAL;
+        }
+        const int64_t kv_len = (int64_t)r.ctx_off + r.q_len;
+        if ((int64_t)r.n_blocks * B < kv_len || kv_len > INT32_MAX) {
+            cp_set_error("cp_build_batch: request %d: block table covers %lld < %lld tokens", j,
+                         (long long)r.n_blocks * B, (long long)kv_len);
+            return CP_EINVAL;
+        }
+        const int used_pages = (int)((kv_len + B - 1) / B);
+        for (int p = 0; p < used_pages; ++p)
+            if (r.block_table[p] < 0 || r.block_table[p] >= c->cfg.num_blocks) {
+                cp_set_error("cp_build_batch: request %d: page id %d out of range", j, r.block_table[p]);
+                return CP_EINVAL;
+            }
+        T += r.q_len;
+        P += used_pages;
+        if (r.q_len == 1) {
+            ++n_decode; f_dec += 1; f_sum_ctx += (float)(r.ctx_off + 1);
+            f_max_ctx = std::max(f_max_ctx, (float)(r.ctx_off + 1));
+        } else {
+            ++n_prefill; f_pf_tokens += (float)r.q_len; f_pf_proc += (float)r.ctx_off;
+            f_pf_proc_max = std::max(f_pf_proc_max, (float)r.ctx_off);
+        }
+        for (int q0 = 0; q0 < r.q_len; q0 += TQ) {
+            const int64_t lim = (int64_t)r.ctx_off + std::min(r.q_len, q0 + TQ);
+            total_tiles += (lim + kKeyTile - 1) / kKeyTile * sh.Hkv;
+        }
+    }
+    if (T > c->cfg.max_tokens) { cp_set_error("cp_build_batch: %lld tokens > max_tokens %d", (long long)T, c->cfg.max_tokens); return CP_ECAPACITY; }
+    if (P > c->cfg.max_total_pages) { cp_set_error("cp_build_batch: %lld pages > max_total_pages %lld", (long long)P, (long long)c->cfg.max_total_pages); return CP_ECAPACITY; }
+
+    // ---- plan: split long key ranges so the persistent grid stays balanced ---------------
+    // ~12 items per SM on average; an item is never longer than total / (12 * n_sm) tiles, so
+    // the LPT-ordered dynamic schedule ends with a short tail.
+    const int64_t per = (int64_t)c->n_sm * 12;
+    int chunk_tiles = (int)std::min<int64_t>(1 << 20, std::max<int64_t>(1, (total_tiles + per - 1) / per));
+    int64_t partial_rows = 0;
+    for (int attempt = 0;; ++attempt) {
+        c->items.clear();
+        c->combines.clear();
+        partial_rows = 0;
+        int64_t tok = 0;
+        bool overflow = false;
+        for (int j = 0; j < n_reqs && !overflow; ++j) {
+            const cp_req_desc& r = reqs[j];
+            for (int q0 = 0; q0 < r.q_len && !overflow; q0 += TQ) {
+                const int qt = std::min(TQ, r.q_len - q0);
+                const int rows = qt * G;
+                const int lim = r.ctx_off + q0 + qt;                 // causal limit of the last row
+                const int n_tiles = (lim + kKeyTile - 1) / kKeyTile;
+                const int n_splits = (n_tiles + chunk_tiles - 1) / chunk_tiles;
+                const int tps = (n_tiles + n_splits - 1) / n_splits;
+                const int kind = (c->use_tc && rows <= 16) ? kKindSwap : kKindTile;
+                for (int g = 0; g < sh.Hkv; ++g) {
+                    int32_t prow = -1;
+                    if (n_splits > 1) {
+                        prow = (int32_t)partial_rows;
+                        partial_rows += (int64_t)n_splits * rows;
+                        if (partial_rows > c->max_partial_rows || partial_rows > INT32_MAX ||
+                            c->combines.size() >= c->max_combine) { overflow = true; break; }
+                        c->combines.push_back(CombineItem{(int32_t)(tok + q0), qt, g, n_splits, prow, {0, 0, 0}});
+                    }
+                    if (c->items.size() + n_splits > c->max_items) { overflow = true; break; }
+                    for (int s = 0; s < n_splits; ++s) {
+                        const int kb = s * tps * kKeyTile;
+                        const int ke = std::min(lim, (s + 1) * tps * kKeyTile);
+                        c->items.push_back(WorkItem{j, g, q0, qt, kb, ke,
+                                                    prow < 0 ? -1 : prow + s * rows, kind});
+                    }
+                }
+            }
+            tok += r.q_len;
+        }
+        if (!overflow) break;
+        if (chunk_tiles >= (1 << 20)) { cp_set_error("cp_build_batch: work list does not fit the limits of cp_create"); return CP_ECAPACITY; }
+        chunk_tiles *= 2;                                            // coarser splits need less workspace
+    }
+
+    // ---- LPT order: bucket sort by descending number of key tiles -------------------------
+    const size_t n_items = c->items.size();
+    int max_cost = 0;
+    for (const WorkItem& w : c->items) max_cost = std::max(max_cost, (w.kv_end - w.kv_begin + kKeyTile - 1) / kKeyTile);
+    c->bucket.assign((size_t)max_cost + 2, 0);
+    for (const WorkItem& w : c->items) ++c->bucket[(size_t)(max_cost - (w.kv_end - w.kv_begin + kKeyTile - 1) / kKeyTile) + 1];
+    for (size_t i = 1; i < c->bucket.size(); ++i) c->bucket[i] += c->bucket[i - 1];
+    c->sorted.resize(n_items);
+    for (const WorkItem& w : c->items) c->sorted[c->bucket[(size_t)(max_cost - (w.kv_end - w.kv_begin + kKeyTile - 1) / kKeyTile)]++] = w;
+
+    // ---- pack into pinned staging ------------------------------------------------------------
+    const int si = c->stage_idx ^ 1;
+    if (c->stage_used[si]) CP_CUDA(cudaEventSynchronize(c->stage_done[si]));   // long since done
+    uint8_t* h = c->h_stage[si];
+    size_t off = 0;
+    auto place = [&](size_t bytes) { size_t o = off; off += align_up(bytes, 16); return o; };
+    const size_t o_cu = place(sizeof(int32_t) * (n_reqs + 1));
+    const size_t o_ql = place(sizeof(int32_t) * n_reqs);
+    const size_t o_co = place(sizeof(int32_t) * n_reqs);
+    const size_t o_bo = place(sizeof(int32_t) * (n_reqs + 1));
+    const size_t o_bt = place(sizeof(int32_t) * (size_t)P);
+    const size_t o_tr = place(sizeof(int32_t) * (size_t)T);
+    const size_t o_wk = place(sizeof(WorkItem) * n_items);
+    const size_t o_cb = place(sizeof(CombineItem) * c->combines.size());
+    if (off > c->meta_cap) { cp_set_error("cp_build_batch: metadata %zu B > capacity %zu B", off, c->meta_cap); return CP_ECAPACITY; }
+    int32_t* cu = reinterpret_cast<int32_t*>(h + o_cu);
+    int32_t* ql = reinterpret_cast<int32_t*>(h + o_ql);
+    int32_t* co = reinterpret_cast<int32_t*>(h + o_co);
+    int32_t* bo = reinterpret_cast<int32_t*>(h + o_bo);
+    int32_t* bt = reinterpret_cast<int32_t*>(h + o_bt);
+    int32_t* tr = reinterpret_cast<int32_t*>(h + o_tr);
+    cu[0] = 0;
+    bo[0] = 0;
+    for (int j = 0; j < n_reqs; ++j) {
+        const cp_req_desc& r = reqs[j];
+        const int used_pages = (int)(((int64_t)r.ctx_off + r.q_len + B - 1) / B);
+        ql[j] = r.q_len;
+        co[j] = r.ctx_off;
+        cu[j + 1] = cu[j] + r.q_len;
+        bo[j + 1] = bo[j] + used_pages;
+        std::memcpy(bt + bo[j], r.block_table, sizeof(int32_t) * used_pages);
+        for (int i = 0; i < r.q_len; ++i) tr[cu[j] + i] = j;
+    }
+    std::memcpy(h + o_wk, c->sorted.data(), sizeof(WorkItem) * n_items);
+    std::memcpy(h + o_cb, c->combines.data(), sizeof(CombineItem) * c->combines.size());
+
+    if (off > 0) CP_CUDA(cudaMemcpyAsync(c->d_meta, h, off, cudaMemcpyHostToDevice, stream));
+    CP_CUDA(cudaEventRecord(c->stage_done[si], stream));
+    c->stage_used[si] = true;
+    c->stage_idx = si;
+
+    BatchMeta& m = c->meta;
+    m.cu_q = reinterpret_cast<const int32_t*>(c->d_meta + o_cu);
+    m.q_len = reinterpret_cast<const int32_t*>(c->d_meta + o_ql);
+    m.ctx_off = reinterpret_cast<const int32_t*>(c->d_meta + o_co);
+    m.bt_off = reinterpret_cast<const int32_t*>(c->d_meta + o_bo);
+    m.block_table = reinterpret_cast<const int32_t*>(c->d_meta + o_bt);
+    m.tok_req = reinterpret_cast<const int32_t*>(c->d_meta + o_tr);
+    m.work = reinterpret_cast<const WorkItem*>(c->d_meta + o_wk);
+    m.combine = reinterpret_cast<const CombineItem*>(c->d_meta + o_cb);
+    m.n_reqs = n_reqs;
+    m.n_tokens = (int32_t)T;
+    m.n_work = (int32_t)n_items;
+    m.n_combine = (int32_t)c->combines.size();
+
+    int32_t n_tc = 0;
+    if (c->use_tc) n_tc = (int32_t)n_items;
+    c->info = cp_batch_info{n_reqs, (int32_t)T, (int32_t)n_items, (int32_t)c->combines.size(), n_tc,
+                            partial_rows, 0, 0, 0};
+    c->feat[0] = f_pf_tokens; c->feat[1] = f_dec; c->feat[2] = (float)n_reqs; c->feat[3] = f_sum_ctx;
+    c->feat[4] = f_max_ctx; c->feat[5] = f_pf_proc; c->feat[6] = f_pf_proc_max;
+    c->n_prefill = n_prefill;
+    c->n_decode = n_decode;
+    c->have_batch = true;
+    ++c->iter;
+    return CP_OK;
+}
+
+// ------------------------------------------------------------------------------------
+// H2-H5: cp_attention_step
+// ------------------------------------------------------------------------------------
+template <int D>
+static int launch_simt(cp_ctx* c, const __nv_bfloat16* q, const __nv_bfloat16* cache,
+                       __nv_bfloat16* out, cudaStream_t stream) {
+    const BatchMeta& m = c->meta;
+    if (m.n_work > 0) {
+        attn_simt_kernel<D><<<m.n_work, 128, 0, stream>>>(m, c->shape, q, cache, out, c->d_part_o, c->d_part_ml);
+        CP_CUDA(cudaGetLastError());
+    }
+    if (m.n_combine > 0) {
+        combine_kernel<D><<<m.n_combine, 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
+        CP_CUDA(cudaGetLastError());
+    }
+    return CP_OK;
+}
+
+extern "C" int cp_attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new,
+                                 const void* v_new, void* kv_cache, void* out, void* stream_) {
+    if (!c) return CP_EINVAL;
+    if (!c->have_batch) { cp_set_error("cp_attention_step: no batch built"); return CP_ESTATE; }
+    if (!q || !kv_cache || !out || ((k_new == nullptr) != (v_new == nullptr)) || layer < 0) {
+        cp_set_error("cp_attention_step: bad argument");
+        return CP_EINVAL;
+    }
+    if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(kv_cache) | reinterpret_cast<uintptr_t>(out) |
+         reinterpret_cast<uintptr_t>(k_new) | reinterpret_cast<uintptr_t>(v_new)) & 15) {
+        cp_set_error("cp_attention_step: pointers must be 16-byte aligned");
+        return CP_EINVAL;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const BatchMeta& m = c->meta;
+    TimedStep& ts = c->ring[(size_t)(c->ring_head % kRing)];
+    CP_CUDA(cudaEventRecord(ts.start, stream));
+    int launches = 0;
+    if (m.n_tokens > 0) {
+        if (k_new) {
+            const int64_t total = (int64_t)m.n_tokens * c->shape.Hkv * (c->shape.D / 8) * 2;
+            const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 8);
+            kv_append_kernel<<<grid, 256, 0, stream>>>(m, c->shape, static_cast<const uint4*>(k_new),
+                                                       static_cast<const uint4*>(v_new),
+                                                       static_cast<__nv_bfloat16*>(kv_cache));
+            CP_CUDA(cudaGetLastError());
+            ++launches;
+        }
+        int rc;
+#ifdef CP_WITH_TC
+        if (c->use_tc) {
+            rc = launch_tc(c, static_cast<const __nv_bfloat16*>(q), static_cast<__nv_bfloat16*>(kv_cache),
+                           static_cast<__nv_bfloat16*>(out), stream, &launches);
+        } else
+#endif
+        {
+            rc = c->shape.D == 128
+                     ? launch_simt<128>(c, static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(kv_cache),
+                                        static_cast<__nv_bfloat16*>(out), stream)
+                     : launch_simt<64>(c, static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(kv_cache),
+                                       static_cast<__nv_bfloat16*>(out), stream);
+            launches += (m.n_work > 0) + (m.n_combine > 0);
+            c->info.grid_attn = m.n_work;
+            c->info.grid_combine = m.n_combine;
+        }
+        if (rc != CP_OK) return rc;
+    }
+    CP_CUDA(cudaEventRecord(ts.stop, stream));
+    c->info.kernels_per_step = launches;
+    cp_latency_row& row = ts.row;
+    std::memcpy(row.feat, c->feat, sizeof(float) * 7);
+    std::memcpy(row.feat + 7, c->mem_stats, sizeof(float) * 4);
+    row.us = 0.f;
+    row.n_prefill = c->n_prefill;
+    row.n_decode = c->n_decode;
+    row.layer = layer;
+    row.iter = c->iter;
+    ++c->ring_head;
+    if (c->ring_head - c->ring_tail > kRing) c->ring_tail = c->ring_head - kRing;   // oldest rows overwritten
+    return CP_OK;
+}
+
+// ------------------------------------------------------------------------------------
+// H6: cp_latency_table
+// ------------------------------------------------------------------------------------
+extern "C" int cp_latency_table(cp_ctx* c, cp_latency_row* rows, int32_t cap, int32_t* n_out) {
+    if (!c || !n_out || (cap > 0 && !rows) || cap < 0) { cp_set_error("cp_latency_table: bad argument"); return CP_EINVAL; }
+    int32_t n = 0;
+    while (c->ring_tail < c->ring_head && n < cap) {
+        TimedStep& ts = c->ring[(size_t)(c->ring_tail % kRing)];
+        CP_CUDA(cudaEventSynchronize(ts.stop));
+        float ms = 0.f;
+        CP_CUDA(cudaEventElapsedTime(&ms, ts.start, ts.stop));
+        ts.row.us = ms * 1000.f;
+        rows[n++] = ts.row;
+        ++c->ring_tail;
+    }
+    *n_out = n;
+    return CP_OK;
+}
+
+extern "C" int cp_set_memory_stats(cp_ctx* c, float used, float freemb, float allocated, float reserved) {
+    if (!c) return CP_EINVAL;
+    c->mem_stats[0] = used; c->mem_stats[1] = freemb; c->mem_stats[2] = allocated; c->mem_stats[3] = reserved;
+    return CP_OK;
+}
+
+extern "C" int cp_get_batch_info(cp_ctx* c, cp_batch_info* info) {
+    if (!c || !info) return CP_EINVAL;
+    if (!c->have_batch) { cp_set_error("cp_get_batch_info: no batch built"); return CP_ESTATE; }
+    *info = c->info;
+    return CP_OK;
+}

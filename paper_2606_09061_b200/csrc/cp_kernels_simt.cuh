@@ -1,0 +1,165 @@
+// cp_kernels_simt.cuh -- plain-ALU kernels of libcp for sm_100a:
+//   kv_append_kernel   H2: scatter the iteration's new K/V rows into their pages
+//   attn_simt_kernel   H3/H4 reference path: one warp per (token, q head) row, online
+//                      softmax in fp32, no tensor cores (kernel_variant = 1; also the
+//                      bisecting aid next to the tcgen05 path)
+//   combine_kernel     H5: LSE merge of split-KV partials -> bf16 out
+// Operation defined in include/cp.h / DESIGN.md section 2.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include "cp_internal.h"
+
+namespace cp {
+
+__device__ __forceinline__ int64_t slab_elem_offset(int64_t page, int kv, int head, int Hkv, int B, int D) {
+    return (((page * 2 + kv) * Hkv + head) * (int64_t)B) * D;
+}
+
+// ---------------------------------------------------------------------------------
+// H2: one thread per 16-byte chunk of a (token, kv head, K|V) row.
+// ---------------------------------------------------------------------------------
+__global__ void kv_append_kernel(BatchMeta meta, Shape sh, const uint4* __restrict__ k_new,
+                                 const uint4* __restrict__ v_new, __nv_bfloat16* __restrict__ cache) {
+    const int chunks = sh.D / 8;                          // 16-byte chunks per row
+    const int64_t total = (int64_t)meta.n_tokens * sh.Hkv * chunks * 2;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        int c = (int)(i % chunks);
+        int64_t r = i / chunks;
+        int kv = (int)(r & 1);
+        r >>= 1;
+        int g = (int)(r % sh.Hkv);
+        int tok = (int)(r / sh.Hkv);
+        int req = meta.tok_req[tok];
+        int pos = meta.ctx_off[req] + (tok - meta.cu_q[req]);
+        int64_t page = meta.block_table[meta.bt_off[req] + pos / sh.B];
+        const uint4* src = (kv ? v_new : k_new) + ((int64_t)tok * sh.Hkv + g) * chunks + c;
+        __nv_bfloat16* dst = cache + slab_elem_offset(page, kv, g, sh.Hkv, sh.B, sh.D) +
+                             (int64_t)(pos % sh.B) * sh.D + c * 8;
+        *reinterpret_cast<uint4*>(dst) = *src;
+    }
+}
+
+// ---------------------------------------------------------------------------------
+// Reference attention: CTA per work item, warp per row, lane owns D/32 dims.
+// Scores are kept in log2 units (q pre-scaled by sm_scale * log2 e).
+// ---------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(128)
+attn_simt_kernel(BatchMeta meta, Shape sh, const __nv_bfloat16* __restrict__ q,
+                 const __nv_bfloat16* __restrict__ cache, __nv_bfloat16* __restrict__ out,
+                 float* __restrict__ part_o, float2* __restrict__ part_ml) {
+    constexpr int EPL = D / 32;                           // elements per lane: 2 or 4
+    const WorkItem it = meta.work[blockIdx.x];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int G = sh.G;
+    const int rows = it.q_tokens * G;
+    const int tok0 = meta.cu_q[it.req] + it.q_start;
+    const int ctx = meta.ctx_off[it.req];
+    const int32_t* bt = meta.block_table + meta.bt_off[it.req];
+    const float qscale = sh.sm_scale * 1.4426950408889634f;
+
+    for (int r = warp; r < rows; r += nwarps) {
+        const int tl = r / G, hg = r % G;
+        const int tok = tok0 + tl;
+        const int h = it.kv_head * G + hg;
+        const int limit = min(it.kv_end, ctx + it.q_start + tl + 1);   // causal, diagonal inclusive
+        float qv[EPL];
+        {
+            const __nv_bfloat16* qp = q + ((int64_t)tok * sh.Hq + h) * D + lane * EPL;
+#pragma unroll
+            for (int e = 0; e < EPL; e += 2) {
+                float2 f = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(qp + e));
+                qv[e] = f.x * qscale;
+                qv[e + 1] = f.y * qscale;
+            }
+        }
+        float m = -INFINITY, l = 0.f, acc[EPL];
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+
+        for (int t = it.kv_begin; t < limit; ++t) {
+            const int64_t page = bt[t / sh.B];
+            const int slot = t % sh.B;
+            const __nv_bfloat16* kp = cache + slab_elem_offset(page, 0, it.kv_head, sh.Hkv, sh.B, D) +
+                                      (int64_t)slot * D + lane * EPL;
+            const __nv_bfloat16* vp = kp + (int64_t)sh.Hkv * sh.B * D;     // V slab follows K slabs
+            float s = 0.f, vv[EPL];
+#pragma unroll
+            for (int e = 0; e < EPL; e += 2) {
+                float2 kf = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(kp + e));
+                float2 vf = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(vp + e));
+                s = fmaf(qv[e], kf.x, s);
+                s = fmaf(qv[e + 1], kf.y, s);
+                vv[e] = vf.x;
+                vv[e + 1] = vf.y;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            const float m_new = fmaxf(m, s);
+            const float alpha = exp2f(m - m_new);          // m = -inf -> 0
+            const float p = exp2f(s - m_new);
+            l = l * alpha + p;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e) acc[e] = acc[e] * alpha + p * vv[e];
+            m = m_new;
+        }
+
+        if (it.partial_row < 0) {
+            const float inv = 1.f / l;
+            __nv_bfloat16* op = out + ((int64_t)tok * sh.Hq + h) * D + lane * EPL;
+#pragma unroll
+            for (int e = 0; e < EPL; e += 2)
+                *reinterpret_cast<__nv_bfloat162*>(op + e) =
+                    __floats2bfloat162_rn(acc[e] * inv, acc[e + 1] * inv);
+        } else {
+            const int64_t pr = (int64_t)it.partial_row + r;
+            float* po = part_o + pr * D + lane * EPL;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e) po[e] = acc[e];
+            if (lane == 0) part_ml[pr] = make_float2(m, l);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------
+// H5: out = sum_s w_s O_s / sum_s w_s l_s, w_s = 2^(m_s - max m).  Warp per row.
+// ---------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(128)
+combine_kernel(BatchMeta meta, Shape sh, const float* __restrict__ part_o,
+               const float2* __restrict__ part_ml, __nv_bfloat16* __restrict__ out) {
+    constexpr int EPL = D / 32;
+    const CombineItem it = meta.combine[blockIdx.x];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int R = it.q_tokens * sh.G;
+    for (int r = warp; r < R; r += nwarps) {
+        float M = -INFINITY;
+        for (int s = 0; s < it.n_splits; ++s)
+            M = fmaxf(M, part_ml[(int64_t)it.partial_row + (int64_t)s * R + r].x);
+        float L = 0.f, acc[EPL];
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+        for (int s = 0; s < it.n_splits; ++s) {
+            const int64_t pr = (int64_t)it.partial_row + (int64_t)s * R + r;
+            const float2 ml = part_ml[pr];
+            const float w = exp2f(ml.x - M);               // empty split: m = -inf -> w = 0
+            L += w * ml.y;
+            const float* po = part_o + pr * D + lane * EPL;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e) acc[e] += w * po[e];
+        }
+        const int tok = it.tok0 + r / sh.G;
+        const int h = it.kv_head * sh.G + r % sh.G;
+        const float inv = 1.f / L;
+        __nv_bfloat16* op = out + ((int64_t)tok * sh.Hq + h) * D + lane * EPL;
+#pragma unroll
+        for (int e = 0; e < EPL; e += 2)
+            *reinterpret_cast<__nv_bfloat162*>(op + e) =
+                __floats2bfloat162_rn(acc[e] * inv, acc[e + 1] * inv);
+    }
+}
+
+}  // namespace cp

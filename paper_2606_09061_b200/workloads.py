@@ -284,3 +284,40 @@ def device_values(spec: BatchSpec, device, seed: Optional[int] = None,
             pool.view(torch.int16).fill_(pv)
     pool[touched] = compact
     return q, k_new, v_new, pool, compact
+
+
+# ----------------------------------------------------------------------------
+# configs[4]: request trace for the scheduler-driven run
+# ----------------------------------------------------------------------------
+def make_trace(n_requests: int = 1000, rate_per_s: float = 8.0, seed: int = 0,
+               short_median: float = 256.0, short_sigma: float = 1.0, long_lo: int = 8192,
+               long_hi: int = 32768, p_long: float = 0.3, out_median: float = 128.0,
+               out_sigma: float = 1.0, out_max: int = 4096):
+    """Poisson arrivals; prompt lengths 70% lognormal(median 256) clipped to [1, 8191]
+    + 30% uniform[8192, 32768]; output lengths lognormal(median 128) clipped to
+    [1, out_max] (BASELINE.json configs[4]; sigma = 1.0 is our reading, R7).
+    Returns int64 arrays (req_id, arrival_us, prompt_len, output_len)."""
+    rng = np.random.default_rng(seed)
+    gaps = rng.exponential(1.0 / rate_per_s, size=n_requests)
+    arrival_us = np.floor(np.cumsum(gaps) * 1e6).astype(np.int64)
+    is_long = rng.random(n_requests) < p_long
+    short = np.clip(np.rint(np.exp(np.log(short_median) + short_sigma * rng.standard_normal(n_requests))),
+                    1, long_lo - 1)
+    longp = rng.integers(long_lo, long_hi + 1, size=n_requests)
+    prompt = np.where(is_long, longp, short).astype(np.int64)
+    out = np.clip(np.rint(np.exp(np.log(out_median) + out_sigma * rng.standard_normal(n_requests))),
+                  1, out_max).astype(np.int64)
+    return np.arange(n_requests, dtype=np.int64), arrival_us, prompt, out
+
+
+def make_apc_trace(n_requests: int = 1000, seed: int = 0, mean_gap_us: float = 2000.0):
+    """The APC-ablation shape: 49:1 short (30-50) : long (200-220) prompts,
+    bursty arrivals."""
+    rng = np.random.default_rng(seed)
+    is_long = (np.arange(n_requests) % 50) == 49
+    prompt = np.where(is_long, rng.integers(200, 221, n_requests), rng.integers(30, 51, n_requests))
+    burst = rng.random(n_requests) < 0.3
+    gaps = np.where(burst, 0.0, rng.exponential(mean_gap_us / 0.7, n_requests))
+    arrival_us = np.floor(np.cumsum(gaps)).astype(np.int64)
+    out = rng.integers(8, 65, n_requests)
+    return np.arange(n_requests, dtype=np.int64), arrival_us, prompt.astype(np.int64), out.astype(np.int64)
