@@ -1,0 +1,319 @@
+#!/usr/bin/env python
+"""bench.py -- mixed-batch paged-attention iteration on B200 (libcp), one JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload b2048] [--impl reference]
+
+A "step" is one pass of the hot path over one synthetic batch:
+H1 cp_build_batch (pack + one H2D of metadata) -> H2 KV append -> H3/H4 attention ->
+H5 combine -> H6 event pair, for one layer.  `value` = tokens/s with Q/K/V and the KV
+pool already resident in HBM; `e2e` = the same through the C ABI with HOST buffers
+(pinned Q/K_new/V_new copied in, `out` copied back, every step).  The workload is
+BASELINE.json configs[2] (token budget 2048, the config the north-star target is quoted
+on); inputs are seeded and synthetic (paper_2606_09061_b200/workloads.py).
+N > 1: replicas only (the path does not shard in scope): each rank
+runs an independent replica, no data-path collective, scaling = weak.
+`--impl reference` times the fp64 CPU oracle (test infrastructure) on the host cores.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_09061_b200 import workloads as wl  # noqa: E402
+
+METRIC = "mixed-batch attention tokens/s (iteration us = 1000*ms_per_step; % of HBM/tensor roofline in roofline.frac)"
+UNIT = "tokens/s"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]),
+                    "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                    "source": "measured"}
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0,
+            "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=lambda: [self.lines.append(l) for l in self.proc.stdout], daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample_rate(spec, q_bits, cache_bits, target_s, seed=0):
+    """Time the fp64 oracle, as it stands, on a bounded seeded sample of (token, head) rows.
+    Returns (equivalent tokens/s for the whole batch, threads, description)."""
+    from oracle import attention as ora
+    rng = np.random.default_rng(seed)
+    tabs = spec.compact_tables()
+    cu = np.concatenate([[0], np.cumsum(spec.q_len)])
+    tok_req = np.repeat(np.arange(spec.n_reqs), spec.q_len)
+    keys_of_tok = spec.ctx_off[tok_req].astype(np.int64) + (np.arange(spec.T) - cu[tok_req]) + 1
+
+    def run(n):
+        tok = rng.integers(0, spec.T, size=n).astype(np.int64)
+        head = rng.integers(0, spec.Hq, size=n).astype(np.int32)
+        t0 = time.perf_counter()
+        ora.attention(q_bits, cache_bits, spec.q_len, spec.ctx_off, tabs, spec.sm_scale, rows=(tok, head))
+        return time.perf_counter() - t0, int(keys_of_tok[tok].sum())
+
+    threads = ora.num_threads()
+    dt, pairs = run(64 * threads)                         # calibration (also warms the pages)
+    n = int(max(64 * threads, min(2_000_000, 64 * threads * target_s / max(dt, 1e-3))))
+    dt, pairs = run(n)
+    total_pairs = spec.causal_pairs() * spec.Hq
+    full_s = dt * total_pairs / max(pairs, 1)
+    desc = (f"{n} seeded (token,head) rows of {spec.T * spec.Hq} ({pairs} of {total_pairs} causal "
+            f"pairs) in {dt:.2f} s; full-batch time extrapolated by the causal-pair ratio")
+    return spec.T / full_s, threads, desc
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def run_ours(args):
+    import torch
+    from paper_2606_09061_b200 import binding, build
+    rank, local_rank, world = dist_env()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device(f"cuda:{local_rank}")
+    build.build()
+    spec = wl.CONFIGS[args.workload](seed=rank)           # replicas: same shape, own seed
+    q, k_new, v_new, pool, compact = wl.device_values(spec, dev)
+    n_pages = int(sum(len(b) for b in spec.block_tables))
+    ctx = binding.Context(spec.Hq, spec.Hkv, spec.D, spec.num_blocks, spec.B, sm_scale=spec.sm_scale,
+                          max_tokens=spec.T, max_reqs=spec.n_reqs, max_total_pages=n_pages,
+                          device=local_rank, kernel_variant=args.variant)
+    descs, keep = binding.make_descs(spec.q_len, spec.ctx_off, spec.block_tables)
+    out = torch.empty((spec.T, spec.Hq, spec.D), device=dev, dtype=torch.bfloat16)
+    free_b, total_b = torch.cuda.mem_get_info(dev)
+    ctx.cp_set_memory_stats((total_b - free_b) / 2**20, free_b / 2**20,
+                            torch.cuda.memory_allocated(dev) / 2**20, torch.cuda.memory_reserved(dev) / 2**20)
+
+    def step():
+        ctx.cp_build_batch(descs=descs, n=spec.n_reqs)
+        ctx.cp_attention_step(0, q, k_new, v_new, pool, out)
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    ctx.cp_latency_table()                                 # drop warm-up rows
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_host0 = time.perf_counter()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    t_host_issue = time.perf_counter() - t_host0
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        ms_total = float(t.item())
+    rows = ctx.cp_latency_table()
+    step_us = np.array([r.us for r in rows], dtype=np.float64)
+    info = ctx.cp_get_batch_info()
+
+    # ---- e2e: same metric through the C ABI with HOST buffers ------------------------------
+    hq, hk, hv_ = (t.cpu().pin_memory() for t in (q, k_new, v_new))
+    hout = torch.empty_like(out, device="cpu").pin_memory()
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k_new), torch.empty_like(v_new)
+
+    def e2e_step():
+        dq.copy_(hq, non_blocking=True); dk.copy_(hk, non_blocking=True); dv.copy_(hv_, non_blocking=True)
+        ctx.cp_build_batch(descs=descs, n=spec.n_reqs)
+        ctx.cp_attention_step(0, dq, dk, dv, pool, out)
+        hout.copy_(out, non_blocking=True)
+
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        e2e_step()
+    e1.record()
+    barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    ctx.cp_latency_table()
+    meta_bytes = 4 * (4 * spec.n_reqs + 2 + n_pages + spec.T) + 32 * (info.n_work_items + info.n_combine_items)
+    h2d = int(hq.numel() * 2 + hk.numel() * 2 + hv_.numel() * 2 + meta_bytes)
+    d2h = int(hout.numel() * 2)
+
+    if rank != 0:
+        ctx.close()
+        return
+    peaks = measured_peaks()
+    ms_per_step = ms_total / args.steps
+    tokens_per_s = world * spec.T * args.steps / (ms_total * 1e-3)
+    # roofline for the step's kernels (append + attention + combine), CUDA events on the launch stream
+    attn_us = float(np.mean(step_us)) if len(step_us) else ms_per_step * 1e3
+    bytes_alg, flops_alg = spec.algorithmic_bytes(), spec.flops()
+    t_hbm = bytes_alg / (peaks["hbm_gbs"] * 1e9)
+    t_tc = flops_alg / (peaks["bf16_tflops_sustained"] * 1e12)
+    bound = "hbm" if t_hbm >= t_tc else "tensor"
+    if bound == "hbm":
+        achieved, peak, runit = bytes_alg / (attn_us * 1e-6) / 1e9, peaks["hbm_gbs"], "GB/s"
+    else:
+        achieved, peak, runit = flops_alg / (attn_us * 1e-6) / 1e12, peaks["bf16_tflops_sustained"], "TFLOP/s"
+    res = {
+        "metric": METRIC, "value": tokens_per_s, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[2] '{spec.name}'" if spec.name == "b2048" else spec.name,
+                   "tokens": spec.T, "requests": spec.n_reqs, "decodes": int((spec.q_len == 1).sum()),
+                   "prefill_chunks": int((spec.q_len > 1).sum()), "sum_kv_len": int(spec.kv_len.sum()),
+                   "pages": n_pages, "pool_pages": spec.num_blocks, "Hq": spec.Hq, "Hkv": spec.Hkv,
+                   "D": spec.D, "block": spec.B, "layers_per_step": 1, "l2": "inputs_exceed_l2 (KV >> 126 MB), no flush",
+                   "parallelism": "replicas" if world > 1 else "single", "kernel_variant": args.variant,
+                   "work_items": info.n_work_items, "combine_items": info.n_combine_items},
+        "clocks": clocks,
+        "e2e": {"value": world * spec.T * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps},
+        "gpu_launches": int(info.kernels_per_step * args.steps),
+        "iteration_us": {"step_incl_build_batch": ms_per_step * 1e3, "attention_step_mean": attn_us,
+                         "attention_step_median": float(np.median(step_us)) if len(step_us) else None,
+                         "attention_step_min": float(step_us.min()) if len(step_us) else None,
+                         "host_issue_per_step": t_host_issue / args.steps * 1e6},
+        "tflops": flops_alg / (attn_us * 1e-6) / 1e12, "gbs": bytes_alg / (attn_us * 1e-6) / 1e9,
+        "roofline": {"bound": bound, "achieved": achieved, "peak": peak, "unit": runit,
+                     "frac": achieved / peak, "traffic": None, "peak_source": peaks["source"],
+                     "kernel": "cp_attention_step kernels (append + attention + combine), mean of CUDA-event pairs",
+                     "algorithmic_bytes": bytes_alg, "algorithmic_flops": flops_alg,
+                     "t_hbm_us": t_hbm * 1e6, "t_tensor_us": t_tc * 1e6,
+                     "frac_nominal_8TBs_2250TF": max(bytes_alg / 8e12, flops_alg / 2.25e15) / (attn_us * 1e-6)},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import attention as ora
+        cache = compact.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        kb = k_new.view(torch.int16).cpu().numpy().view(np.uint16)
+        vb = v_new.view(torch.int16).cpu().numpy().view(np.uint16)
+        qb = q.view(torch.int16).cpu().numpy().view(np.uint16)
+        ora.kv_append(kb, vb, cache, spec.q_len, spec.ctx_off, spec.compact_tables())
+        v, threads, desc = oracle_sample_rate(spec, qb, cache, args.cpu_seconds)
+        res["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+    ctx.close()
+    print(json.dumps(res), flush=True)
+
+
+def run_reference(args):
+    """The reference arm for this tier = the fp64 oracle on the host cores (rank 0 only)."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    from oracle import attention as ora
+    spec = wl.CONFIGS[args.workload](seed=0)
+    try:
+        import torch
+        assert torch.cuda.is_available()
+        q, k_new, v_new, pool, compact = wl.device_values(spec, torch.device("cuda:0"))
+        b = lambda t: t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        qb, kb, vb, cache = b(q), b(k_new), b(v_new), b(compact)
+        del pool, compact
+        torch.cuda.empty_cache()
+    except Exception:
+        hv = wl.host_values(spec)
+        qb, kb, vb, cache = hv.q, hv.k_new, hv.v_new, hv.cache
+    ora.kv_append(kb, vb, cache, spec.q_len, spec.ctx_off, spec.compact_tables())
+    per_step_s = max(2.0, min(20.0, 120.0 / (args.steps + args.warmup)))
+    vals, descs, threads = [], [], 1
+    for i in range(args.warmup + args.steps):
+        v, threads, desc = oracle_sample_rate(spec, qb, cache, per_step_s, seed=i)
+        if i >= args.warmup:
+            vals.append(v); descs.append(desc)
+    v = float(np.mean(vals))
+    res = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": spec.T / v * 1e3,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "config": {"workload": spec.name, "tokens": spec.T, "requests": spec.n_reqs},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": descs[-1]},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(res), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="b2048", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--variant", type=int, default=0, help="cp_config.kernel_variant")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

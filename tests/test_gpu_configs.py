@@ -1,0 +1,61 @@
+"""-m gpu parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+configs[1] (budget 512) is compared in full; configs[2] (budget 2048, the target) and
+configs[3] (70B-shaped) on seeded samples of rows the oracle computes one by one."""
+import numpy as np
+import pytest
+
+from oracle import attention as ora
+from paper_2606_09061_b200 import workloads as wl
+from tests import gpu_util as gu
+
+pytestmark = pytest.mark.gpu
+
+
+def _run_device_config(spec, variant, n_sample):
+    import torch
+    dev = torch.device("cuda:0")
+    q, k_new, v_new, pool, compact = wl.device_values(spec, dev)
+    ctx = gu.make_ctx(spec, variant)
+    out = torch.full((spec.T, spec.Hq, spec.D), float("nan"), device=dev, dtype=torch.bfloat16)
+    ctx.cp_build_batch(spec.q_len, spec.ctx_off, spec.block_tables)
+    ctx.cp_attention_step(0, q, k_new, v_new, pool, out)
+    torch.cuda.synchronize()
+    got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)
+    assert np.isfinite(got).all()
+    # oracle: same bits, its own append, sampled rows
+    cache = gu.to_bits(compact)
+    tabs = spec.compact_tables()
+    ora.kv_append(gu.to_bits(k_new), gu.to_bits(v_new), cache, spec.q_len, spec.ctx_off, tabs)
+    # H2 parity: the pages the step wrote equal the oracle's append, bit for bit
+    touched = torch.from_numpy(spec.touched_pages().astype(np.int64)).to(dev)
+    step = 8192
+    for s in range(0, len(touched), step):
+        assert np.array_equal(gu.to_bits(pool[touched[s:s + step]]), cache[s:s + step])
+    if n_sample is None:
+        want = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale)
+        stats = gu.assert_close(got, want, spec.name)
+    else:
+        tok, head = gu.sample_rows(spec, n_sample)
+        want = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale,
+                             rows=(tok, head))
+        stats = gu.assert_close(got[tok, head], want, spec.name)
+    info = ctx.cp_get_batch_info()
+    ctx.close()
+    del pool, compact
+    torch.cuda.empty_cache()
+    return stats, info
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config_b512_full(variant):
+    _run_device_config(wl.config_b512(), variant, None)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config_b2048_sampled(variant):
+    stats, info = _run_device_config(wl.config_b2048(), variant, 2048)
+    assert info.n_tokens == 2048 and info.n_reqs == 516
+
+
+def test_config_70b_sampled():
+    _run_device_config(wl.config_70b(), 0, 1024)

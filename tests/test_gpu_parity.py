@@ -1,0 +1,163 @@
+"""-m gpu parity tests: libcp (through the C ABI) vs the fp64 oracle on the same seeded
+inputs.  Tolerance: max-abs 2e-2 and mean-abs 2e-3 on bf16 outputs (BASELINE.json)."""
+import numpy as np
+import pytest
+
+from oracle import attention as ora
+from paper_2606_09061_b200 import binding, workloads as wl
+from tests import gpu_util as gu
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = [0, 1]       # 0 = default path (tensor-core where built), 1 = SIMT reference kernels
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_tiny_config_full(variant):
+    spec = wl.config_tiny()
+    hv = wl.host_values(spec)
+    got, pool_after = gu.run_gpu_host_values(spec, hv, variant)
+    want, cache_after = gu.run_oracle_host_values(spec, hv)
+    gu.assert_close(got, want, "tiny")
+    # H2: the appended pages are bit-identical to the oracle's append; nothing else moved
+    assert np.array_equal(pool_after[spec.touched_pages()], cache_after)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("seed,Hq,Hkv,D", [(1, 8, 2, 64), (2, 8, 8, 128), (3, 16, 2, 128),
+                                           (4, 16, 1, 64), (5, 4, 2, 128), (6, 32, 8, 128)])
+def test_random_mixed_batches(variant, seed, Hq, Hkv, D):
+    spec = wl.random_spec(seed, Hq=Hq, Hkv=Hkv, D=D, n_prefill=4, n_decode=6, max_chunk=300,
+                          max_ctx=700)
+    hv = wl.host_values(spec)
+    got, _ = gu.run_gpu_host_values(spec, hv, variant)
+    want, _ = gu.run_oracle_host_values(spec, hv)
+    gu.assert_close(got, want, spec.name)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_edge_shapes(variant):
+    # single key; chunk lengths around the tile sizes; offsets around tile/page boundaries
+    q_len = [1, 1, 1, 127, 128, 129, 33, 16, 1, 257]
+    ctx_off = [0, 15, 16, 0, 1, 127, 128, 255, 511, 3]
+    spec = wl.make_spec("edges", 8, 2, 128, 16, 400, q_len, ctx_off, seed=3)
+    hv = wl.host_values(spec)
+    got, _ = gu.run_gpu_host_values(spec, hv, variant)
+    want, _ = gu.run_oracle_host_values(spec, hv)
+    gu.assert_close(got, want, "edges")
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_caller_wrote_pages_path_and_stale_tails(variant):
+    spec = wl.random_spec(11, Hq=8, Hkv=2, D=128)
+    hv = wl.host_values(spec)
+    want, _ = gu.run_oracle_host_values(spec, hv)
+    got, _ = gu.run_gpu_host_values(spec, hv, variant, append=False)
+    gu.assert_close(got, want, "k_new=NULL")
+    # different stale data in tails / untouched pages must not change a single output bit
+    got2, _ = gu.run_gpu_host_values(spec, hv, variant, append=False, poison=wl.POISON_BF16_NEG)
+    assert np.array_equal(got, got2)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_chunking_invariance_and_decode_consistency_on_gpu(variant):
+    """A prompt processed as chunks equals the unchunked prompt (within 2x tolerance GPU vs
+    GPU, within tolerance vs the oracle); a decode equals the last row of full attention."""
+    import torch
+    rng = np.random.default_rng(5)
+    L, Hq, Hkv, D, B = 300, 8, 2, 128, 16
+    Kb = wl.f32_to_bf16_bits(rng.standard_normal((L, Hkv, D), dtype=np.float32))
+    Vb = wl.f32_to_bf16_bits(rng.standard_normal((L, Hkv, D), dtype=np.float32))
+    Qb = wl.f32_to_bf16_bits(rng.standard_normal((L, Hq, D), dtype=np.float32))
+    nb = (L + B - 1) // B
+    bt = rng.permutation(nb + 6)[:nb].astype(np.int32)
+    spec1 = wl.BatchSpec("whole", Hq, Hkv, D, B, nb + 6, np.array([L], np.int32), np.array([0], np.int32), [bt])
+    ctx = gu.make_ctx(spec1, variant, max_tokens=L, max_reqs=4)
+
+    def run(cuts):
+        pool = gu.torch_bf16(np.full((nb + 6, 2, Hkv, B, D), wl.POISON_BF16, np.uint16))
+        outs = []
+        for a, b in zip(cuts[:-1], cuts[1:]):
+            out = torch.empty((b - a, Hq, D), device="cuda", dtype=torch.bfloat16)
+            ctx.cp_build_batch([b - a], [a], [bt])
+            ctx.cp_attention_step(0, gu.torch_bf16(Qb[a:b]), gu.torch_bf16(Kb[a:b]), gu.torch_bf16(Vb[a:b]), pool, out)
+            outs.append(wl.bf16_bits_to_f64(gu.to_bits(out)))
+        return np.concatenate(outs), pool
+
+    whole, pool = run([0, L])
+    chunked, _ = run([0, 1, 2, 50, 128, 129, 177, 290, L])
+    cache = np.full((nb + 6, 2, Hkv, B, D), wl.POISON_BF16, np.uint16)
+    ora.kv_append(Kb, Vb, cache, [L], [0], [bt])
+    want = ora.attention(Qb, cache, [L], [0], [bt], spec1.sm_scale)
+    gu.assert_close(whole, want, "unchunked")
+    gu.assert_close(chunked, want, "chunked")
+    assert np.abs(whole - chunked).max() <= 2 * gu.MAX_ABS_TOL
+    # decode consistency: q of the last token as a decode over the full cache
+    out = torch.empty((1, Hq, D), device="cuda", dtype=torch.bfloat16)
+    ctx.cp_build_batch([1], [L - 1], [bt])
+    ctx.cp_attention_step(0, gu.torch_bf16(Qb[L - 1:]), None, None, pool, out)
+    dec = wl.bf16_bits_to_f64(gu.to_bits(out))
+    gu.assert_close(dec, want[L - 1:], "decode = last row")
+    ctx.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_closed_form_constant_v(variant):
+    spec = wl.random_spec(21, Hq=8, Hkv=2, D=64)
+    hv = wl.host_values(spec)
+    vrow = wl.f32_to_bf16_bits(np.random.default_rng(0).standard_normal((1, spec.Hkv, spec.D), dtype=np.float32))
+    hv.v_new[:] = vrow
+    base = 0
+    for bt, off in zip(spec.block_tables, spec.ctx_off):
+        for pi in range(len(bt)):
+            n_valid = min(max(int(off) - pi * spec.B, 0), spec.B)
+            hv.cache[base + pi, 1, :, :n_valid, :] = vrow[0][:, None, :]
+        base += len(bt)
+    got, _ = gu.run_gpu_host_values(spec, hv, variant)
+    G = spec.Hq // spec.Hkv
+    want = np.repeat(wl.bf16_bits_to_f64(vrow)[0], G, axis=0)[None]
+    assert np.abs(got - want).max() <= 2 ** -8 * np.abs(want).max()      # one bf16 rounding
+
+
+def test_empty_batch_and_errors():
+    import torch
+    spec = wl.config_tiny()
+    ctx = gu.make_ctx(spec, 1, max_tokens=64, max_reqs=4, max_total_pages=16)
+    with pytest.raises(binding.CpError) as e:
+        ctx.cp_attention_step(0, 16, None, None, 16, 16)
+    assert e.value.code == binding.CP_ESTATE
+    ctx.cp_build_batch([], [], [])
+    dummy = torch.zeros(64, device="cuda", dtype=torch.bfloat16)
+    ctx.cp_attention_step(0, dummy, None, None, dummy, dummy)           # no-op, still timed
+    torch.cuda.synchronize()
+    for q, o, bt, code in [([0], [0], [[0]], binding.CP_EINVAL), ([1], [-1], [[0]], binding.CP_EINVAL),
+                           ([17], [0], [[0]], binding.CP_EINVAL), ([1], [0], [[16]], binding.CP_EINVAL),
+                           ([65], [0], [[0, 1, 2, 3, 4]], binding.CP_ECAPACITY),
+                           ([1] * 5, [0] * 5, [[i] for i in range(5)], binding.CP_ECAPACITY)]:
+        with pytest.raises(binding.CpError) as e:
+            ctx.cp_build_batch(q, o, [np.asarray(b, np.int32) for b in bt])
+        assert e.value.code == code
+    assert ctx.cp_get_batch_info().n_reqs == 0          # failed builds kept the previous batch
+    ctx.close()
+
+
+def test_latency_table_rows():
+    import torch
+    spec = wl.config_tiny()
+    hv = wl.host_values(spec)
+    ctx = gu.make_ctx(spec, 0, num_layers=3)
+    ctx.cp_set_memory_stats(10.0, 20.0, 5.0, 8.0)
+    pool = gu.torch_bf16(wl.full_pool_from_compact(spec, hv.cache))
+    out = torch.empty((spec.T, spec.Hq, spec.D), device="cuda", dtype=torch.bfloat16)
+    ctx.cp_build_batch(spec.q_len, spec.ctx_off, spec.block_tables)
+    for layer in range(3):
+        ctx.cp_attention_step(layer, gu.torch_bf16(hv.q), None if layer else gu.torch_bf16(hv.k_new),
+                              None if layer else gu.torch_bf16(hv.v_new), pool, out)
+    rows = ctx.cp_latency_table()
+    assert [r.layer for r in rows] == [0, 1, 2] and all(r.us > 0 for r in rows)
+    r = rows[0]
+    # Table 1 features of this batch: chunks (32 @0), (16 @48); decodes ctx 40, 100
+    assert list(r.feat) == [48.0, 2.0, 4.0, 140.0, 100.0, 48.0, 48.0, 10.0, 20.0, 5.0, 8.0]
+    assert (r.n_prefill, r.n_decode, r.iter) == (2, 2, 0)
+    assert ctx.cp_latency_table() == []
+    ctx.close()
