@@ -1,5 +1,6 @@
 // cp_api.cu -- libcp's C ABI for the GPU path: context, batch packing (H1), the attention
 // step launcher (H2-H5) and the latency table (H6).  See include/cp.h for the contract.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -77,6 +78,11 @@ struct cp_ctx {
     std::vector<WorkItem> items, sorted;
     std::vector<CombineItem> combines;
     std::vector<int32_t> bucket;
+
+    // tensor-core path: one TMA descriptor per KV pool pointer (one per layer), encoded once
+    std::vector<std::pair<const void*, CUtensorMap>> tmaps;
+    void* encode_fn = nullptr;
+    bool tc_attr_set = false;
 };
 
 extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
@@ -242,7 +248,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
                 const int n_tiles = (lim + kKeyTile - 1) / kKeyTile;
                 const int n_splits = (n_tiles + chunk_tiles - 1) / chunk_tiles;
                 const int tps = (n_tiles + n_splits - 1) / n_splits;
-                const int kind = (c->use_tc && rows <= 16) ? kKindSwap : kKindTile;
+                const int kind = (c->use_tc && rows <= 16 && sh.D == 128) ? kKindSwap : kKindTile;
                 for (int g = 0; g < sh.Hkv; ++g) {
                     int32_t prow = -1;
                     if (n_splits > 1) {
@@ -363,6 +369,76 @@ static int launch_simt(cp_ctx* c, const __nv_bfloat16* q, const __nv_bfloat16* c
     }
     return CP_OK;
 }
+
+#ifdef CP_WITH_TC
+typedef CUresult (*cuTensorMapEncodeTiled_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                             const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                             CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                             CUtensorMapFloatOOBfill);
+
+// The KV pool as a 3-D bf16 tensor {D, B, slabs} (slab = (block, K|V, kv head)); one box =
+// 64 elements x 16 tokens of one slab = 2 KiB, written with the 128-byte swizzle UMMA expects.
+static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out) {
+    for (auto& e : c->tmaps)
+        if (e.first == kv_cache) { *out = &e.second; return CP_OK; }
+    if (!c->encode_fn) {
+        cudaDriverEntryPointQueryResult qres;
+        CP_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &c->encode_fn, cudaEnableDefault, &qres));
+        if (qres != cudaDriverEntryPointSuccess || !c->encode_fn) {
+            cp_set_error("cuTensorMapEncodeTiled not available from the driver");
+            return CP_ECUDA;
+        }
+    }
+    const Shape& sh = c->shape;
+    CUtensorMap m;
+    const cuuint64_t dims[3] = {(cuuint64_t)sh.D, (cuuint64_t)sh.B, (cuuint64_t)c->cfg.num_blocks * 2 * sh.Hkv};
+    const cuuint64_t strides[2] = {(cuuint64_t)sh.D * 2, (cuuint64_t)sh.D * sh.B * 2};
+    const cuuint32_t box[3] = {64, (cuuint32_t)sh.B, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = reinterpret_cast<cuTensorMapEncodeTiled_t>(c->encode_fn)(
+        &m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kv_cache, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { cp_set_error("cuTensorMapEncodeTiled failed: %d", (int)r); return CP_ECUDA; }
+    if (c->tmaps.size() >= 256) c->tmaps.clear();
+    c->tmaps.emplace_back(kv_cache, m);
+    *out = &c->tmaps.back().second;
+    return CP_OK;
+}
+
+template <int D>
+static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_bfloat16* out, cudaStream_t stream,
+                       int* launches) {
+    const BatchMeta& m = c->meta;
+    const CUtensorMap* tmap = nullptr;
+    int rc = get_tmap(c, kv_cache, &tmap);
+    if (rc != CP_OK) return rc;
+    if (!c->tc_attr_set) {
+        CP_CUDA(cudaFuncSetAttribute(attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcLayout<D>::kTotal));
+        c->tc_attr_set = true;
+    }
+    if (m.n_work > 0) {
+        TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter};
+        const int grid = std::min(c->n_sm, m.n_work);
+        attn_tc_kernel<D><<<grid, kTcThreads, TcLayout<D>::kTotal, stream>>>(p, *tmap);
+        CP_CUDA(cudaGetLastError());
+        ++*launches;
+        c->info.grid_attn = grid;
+    }
+    if (m.n_combine > 0) {
+        combine_kernel<D><<<m.n_combine, 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
+        CP_CUDA(cudaGetLastError());
+        ++*launches;
+    }
+    c->info.grid_combine = m.n_combine;
+    return CP_OK;
+}
+
+static int launch_tc(cp_ctx* c, const __nv_bfloat16* q, __nv_bfloat16* kv_cache, __nv_bfloat16* out,
+                     cudaStream_t stream, int* launches) {
+    return c->shape.D == 128 ? launch_tc_d<128>(c, q, kv_cache, out, stream, launches)
+                             : launch_tc_d<64>(c, q, kv_cache, out, stream, launches);
+}
+#endif
 
 extern "C" int cp_attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new,
                                  const void* v_new, void* kv_cache, void* out, void* stream_) {
