@@ -41,6 +41,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         nv.append("-DCP_WITH_TC")
     if verbose:
         nv += ["-Xptxas", "-v"]
+    nv += os.environ.get("CP_EXTRA_NVCC", "").split()
     objs = []
     cmds = [
         ["nvcc", *nv, "-c", os.path.join(CSRC, "cp_api.cu"), "-o", os.path.join(OBJ, "cp_api.o")],

@@ -55,6 +55,7 @@ struct cp_ctx {
     float* d_part_o = nullptr;
     float2* d_part_ml = nullptr;
     int32_t* d_counter = nullptr;      // persistent-kernel work counter
+    unsigned long long* d_prof = nullptr;   // CP_TC_PROF builds only
     // pinned staging, double buffered
     uint8_t* h_stage[2] = {nullptr, nullptr};
     cudaEvent_t stage_done[2] = {nullptr, nullptr};
@@ -136,6 +137,10 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     chk(cudaMalloc(&c->d_part_o, sizeof(float) * (size_t)c->max_partial_rows * D));
     chk(cudaMalloc(&c->d_part_ml, sizeof(float2) * (size_t)c->max_partial_rows));
     chk(cudaMalloc(&c->d_counter, sizeof(int32_t) * 4));
+#if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
+    chk(cudaMalloc(&c->d_prof, sizeof(unsigned long long) * 16 * 1024));
+    chk(cudaMemset(c->d_prof, 0, sizeof(unsigned long long) * 16 * 1024));
+#endif
     chk(cudaMemset(c->d_counter, 0, sizeof(int32_t) * 4));
     for (int i = 0; i < 2; ++i) {
         chk(cudaMallocHost(&c->h_stage[i], cap));
@@ -166,6 +171,7 @@ extern "C" int cp_destroy(cp_ctx* c) {
     cudaFree(c->d_part_o);
     cudaFree(c->d_part_ml);
     cudaFree(c->d_counter);
+    cudaFree(c->d_prof);
     for (int i = 0; i < 2; ++i) {
         if (c->h_stage[i]) cudaFreeHost(c->h_stage[i]);
         if (c->stage_done[i]) cudaEventDestroy(c->stage_done[i]);
@@ -376,8 +382,7 @@ typedef CUresult (*cuTensorMapEncodeTiled_t)(CUtensorMap*, CUtensorMapDataType, 
                                              CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
                                              CUtensorMapFloatOOBfill);
 
-// The KV pool as a 3-D bf16 tensor {D, B, slabs} (slab = (block, K|V, kv head)); one box =
-// 64 elements x 16 tokens of one slab = 2 KiB, written with the 128-byte swizzle UMMA expects.
+// TMA descriptor of one layer's KV pool (slab = (block, K|V, kv head)), 128-byte swizzle.
 static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out) {
     for (auto& e : c->tmaps)
         if (e.first == kv_cache) { *out = &e.second; return CP_OK; }
@@ -391,12 +396,19 @@ static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out) {
     }
     const Shape& sh = c->shape;
     CUtensorMap m;
-    const cuuint64_t dims[3] = {(cuuint64_t)sh.D, (cuuint64_t)sh.B, (cuuint64_t)c->cfg.num_blocks * 2 * sh.Hkv};
-    const cuuint64_t strides[2] = {(cuuint64_t)sh.D * 2, (cuuint64_t)sh.D * sh.B * 2};
-    const cuuint32_t box[3] = {64, (cuuint32_t)sh.B, 1};
-    const cuuint32_t estr[3] = {1, 1, 1};
+    // 5-D view of the pool so that ONE box = one whole (block, K|V, head) slab of 16 tokens x D:
+    //   d0 64 elements (one 128-byte half-row)     d1 8 tokens of a row group (stride D*2)
+    //   d2 D/64 halves of a row (stride 128 B)     d3 2 row groups (stride 8*D*2)
+    //   d4 slab index (stride 16*D*2)
+    // The box lands in smem as [row group][half][8 rows][128 B]: 8-row groups of each half are
+    // D/64 KiB apart for the whole 128-key tile, which is a legal UMMA SBO (see cp_kernels_tc.cuh).
+    const cuuint64_t rowb = (cuuint64_t)sh.D * 2;
+    const cuuint64_t dims[5] = {64, 8, (cuuint64_t)sh.D / 64, 2, (cuuint64_t)c->cfg.num_blocks * 2 * sh.Hkv};
+    const cuuint64_t strides[4] = {rowb, 128, 8 * rowb, 16 * rowb};
+    const cuuint32_t box[5] = {64, 8, (cuuint32_t)sh.D / 64, 2, 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     CUresult r = reinterpret_cast<cuTensorMapEncodeTiled_t>(c->encode_fn)(
-        &m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, kv_cache, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+        &m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, kv_cache, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { cp_set_error("cuTensorMapEncodeTiled failed: %d", (int)r); return CP_ECUDA; }
     if (c->tmaps.size() >= 256) c->tmaps.clear();
@@ -417,7 +429,7 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
         c->tc_attr_set = true;
     }
     if (m.n_work > 0) {
-        TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter};
+        TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
         const int grid = std::min(c->n_sm, m.n_work);
         attn_tc_kernel<D><<<grid, kTcThreads, TcLayout<D>::kTotal, stream>>>(p, *tmap);
         CP_CUDA(cudaGetLastError());
@@ -526,6 +538,15 @@ extern "C" int cp_set_memory_stats(cp_ctx* c, float used, float freemb, float al
     c->mem_stats[0] = used; c->mem_stats[1] = freemb; c->mem_stats[2] = allocated; c->mem_stats[3] = reserved;
     return CP_OK;
 }
+
+#if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
+// debug builds only (not part of include/cp.h): per-CTA wait-time profile of the last launch
+extern "C" int cp_debug_prof(cp_ctx* c, unsigned long long* host_buf, int n_ctas) {
+    if (!c->d_prof) return CP_ESTATE;
+    cudaDeviceSynchronize();
+    return cudaMemcpy(host_buf, c->d_prof, sizeof(unsigned long long) * 16 * n_ctas, cudaMemcpyDeviceToHost) == cudaSuccess ? CP_OK : CP_ECUDA;
+}
+#endif
 
 extern "C" int cp_get_batch_info(cp_ctx* c, cp_batch_info* info) {
     if (!c || !info) return CP_EINVAL;

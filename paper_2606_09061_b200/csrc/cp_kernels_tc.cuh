@@ -31,6 +31,7 @@ namespace cp {
 constexpr int kTcThreads = 192;
 constexpr int kStages = 5;
 constexpr int kTmemCols = 512;
+constexpr int kItemRing = 2;
 constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO = 256;
 constexpr float kRescaleThreshold = 8.0f;      // log2 units: rescale O only when the max grew > 2^8
 
@@ -41,13 +42,36 @@ struct TcLayout {
     static constexpr uint32_t kQBytes = kHalves * kHalfBytes;
     static constexpr uint32_t kPBytes = 2 * kHalfBytes;    // 128 rows x 128 keys bf16
     static constexpr uint32_t kSlotBytes = kHalves * kHalfBytes;
+    // K/V slot: [16 row groups][kHalves][8 rows][128 B] (one TMA box per page = 2 row groups)
+    static constexpr uint32_t kGroupBytes = kHalves * 1024;   // UMMA SBO of a K/V slot
+    static constexpr uint32_t kPageBytes = 2 * kGroupBytes;
     static constexpr uint32_t kOffQ = 0;
     static constexpr uint32_t kOffP = kQBytes;
     static constexpr uint32_t kOffKV = kOffP + kPBytes;
     static constexpr uint32_t kOffMisc = kOffKV + kStages * kSlotBytes;
-    static constexpr uint32_t kMiscBytes = 1024;
+    static constexpr uint32_t kMiscBytes = 2048;
     static constexpr uint32_t kTotal = kOffMisc + kMiscBytes + 1024;   // + slack to align the base to 1024
 };
+
+// Optional role-level wait-time profile (build with -DCP_TC_PROF; debugging aid only).
+#ifdef CP_TC_PROF2
+#define CP_STAMP(id) do { if (threadIdx.x == 128) { long long t__ = clock64(); misc->prof[id] += (unsigned long long)(t__ - tprev__); tprev__ = t__; } } while (0)
+#define CP_STAMP_INIT long long tprev__ = clock64()
+#else
+#define CP_STAMP(id) do {} while (0)
+#define CP_STAMP_INIT do {} while (0)
+#endif
+#ifdef CP_TC_PROF
+#define CP_PWAIT(id, bar, par)                                                        \
+    do {                                                                              \
+        const long long t0__ = clock64();                                             \
+        ptx::mbar_wait(bar, par);                                                     \
+        if ((threadIdx.x & 31) == 0 && (threadIdx.x < 64 || threadIdx.x == 128))      \
+            misc->prof[id] += (unsigned long long)(clock64() - t0__);                 \
+    } while (0)
+#else
+#define CP_PWAIT(id, bar, par) ptx::mbar_wait(bar, par)
+#endif
 
 struct TcMisc {                 // lives in the misc region
     uint64_t kv_full[kStages];
@@ -55,13 +79,18 @@ struct TcMisc {                 // lives in the misc region
     uint64_t q_full;
     uint64_t s_full[2];
     uint64_t p_full;
-    uint64_t pv_done;
+    uint64_t pv_done[2];        // PV of tile gt completes on pv_done[gt & 1]
+    uint64_t item_full[kItemRing];
+    uint64_t item_empty[kItemRing];
+    WorkItem items[kItemRing];  // published by the producer warp; kind < 0 = no more work
     uint32_t tmem_base;
-    int32_t item;
+#if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
+    unsigned long long prof[16];
+#endif
     float cmax[2][4][16];       // swap path: per-warp column maxima, double buffered
     float lsum[4][16];          // swap path: per-warp column sums at the end of an item
 };
-static_assert(sizeof(TcMisc) <= 1024, "misc region too small");
+static_assert(sizeof(TcMisc) <= 2048, "misc region too small");
 
 struct TcParams {
     BatchMeta meta;
@@ -71,6 +100,7 @@ struct TcParams {
     float* part_o;
     float2* part_ml;
     int32_t* counters;          // [0] next item, [1] finished CTAs
+    unsigned long long* prof;   // [grid][16] wait-time profile (CP_TC_PROF builds), else unused
 };
 
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
@@ -79,39 +109,74 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 }
 
 // ------------------------------------------------------------------------------------------
-// producer: stream the K and V tiles of one item into the slot ring, in consumption order
-//   K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1)
+// producer warp: fetches work items (atomic counter), publishes them to the other roles through
+// a small smem ring, and streams the K and V tiles of each item into the slot ring in
+// consumption order  K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1).  It runs ahead of the
+// consumers by up to kStages tile loads, across item boundaries.  Page ids are prefetched 32 at
+// a time (one per lane) so no dependent global load sits between two TMA issues.
 // ------------------------------------------------------------------------------------------
 template <int D>
-__device__ __forceinline__ void tc_produce_item(const WorkItem& it, const BatchMeta& meta, const Shape& sh,
-                                                const CUtensorMap* tmap, uint8_t* kv_base, TcMisc* misc,
-                                                uint32_t& ld_cnt, int lane) {
+__device__ __forceinline__ void tc_producer(const TcParams& p, const CUtensorMap* tmap, uint8_t* kv_base,
+                                            TcMisc* misc, int lane) {
     using L = TcLayout<D>;
-    const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
-    const int32_t* bt = meta.block_table + meta.bt_off[it.req];
-    for (int i = 0; i < 2 * n_tiles; ++i) {
-        int is_v, tile;
-        if (i == 0) { is_v = 0; tile = 0; }
-        else if (i == 2 * n_tiles - 1) { is_v = 1; tile = n_tiles - 1; }
-        else if (i & 1) { is_v = 0; tile = (i + 1) >> 1; }
-        else { is_v = 1; tile = (i >> 1) - 1; }
-        const int ts = it.kv_begin + tile * kKeyTile;
-        const int n_pages = (min(it.kv_end, ts + kKeyTile) - ts + 15) >> 4;     // 1..8
-        const uint32_t slot = ld_cnt % kStages;
-        const uint32_t parity = ((ld_cnt / kStages) & 1) ^ 1;
-        ptx::mbar_wait(&misc->kv_empty[slot], parity);
-        if (lane == 0) ptx::mbar_arrive_expect_tx(&misc->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u);
+    uint32_t ld_cnt = 0, item_cnt = 0;
+    for (;;) {
+        int idx = 0;
+        if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
+        idx = __shfl_sync(0xffffffffu, idx, 0);
+        const bool done = idx >= p.meta.n_work;
+        // one int32 of the 32-byte WorkItem per lane 0..7
+        int w = 0;
+        if (!done && lane < 8) w = reinterpret_cast<const int32_t*>(p.meta.work + idx)[lane];
+        if (done && lane == 7) w = -1;                                   // kind = -1: sentinel
+        const uint32_t islot = item_cnt % kItemRing;
+        CP_PWAIT(0, &misc->item_empty[islot], ((item_cnt / kItemRing) & 1) ^ 1);
+        if (lane < 8) reinterpret_cast<int32_t*>(&misc->items[islot])[lane] = w;
         __syncwarp();
-        if (lane < n_pages) {
-            const int page = bt[(ts >> 4) + lane];
-            const int slab = (page * 2 + is_v) * sh.Hkv + it.kv_head;
-            uint8_t* dst = kv_base + slot * L::kSlotBytes + lane * 2048;
+        if (lane == 0) ptx::mbar_arrive(&misc->item_full[islot]);
+        ++item_cnt;
+        if (done) break;
+        const int req = __shfl_sync(0xffffffffu, w, 0), kv_head = __shfl_sync(0xffffffffu, w, 1);
+        const int kv_begin = __shfl_sync(0xffffffffu, w, 4), kv_end = __shfl_sync(0xffffffffu, w, 5);
+        const int n_tiles = (kv_end - kv_begin + kKeyTile - 1) / kKeyTile;
+        const int32_t* bt = p.meta.block_table + p.meta.bt_off[req] + (kv_begin >> 4);
+        const int n_pages_item = (kv_end - kv_begin + 15) >> 4;
+        // page-id windows of 32 pages (4 tiles): cur = window cur_w, nxt = window cur_w + 1
+        int cur_w = 0;
+        int cur = lane < n_pages_item ? bt[lane] : 0;
+        int nxt = 32 + lane < n_pages_item ? bt[32 + lane] : 0;
+        for (int i = 0; i < 2 * n_tiles; ++i) {
+            int is_v, tile;
+            if (i == 0) { is_v = 0; tile = 0; }
+            else if (i == 2 * n_tiles - 1) { is_v = 1; tile = n_tiles - 1; }
+            else if (i & 1) { is_v = 0; tile = (i + 1) >> 1; }
+            else { is_v = 1; tile = (i >> 1) - 1; }
+            if ((tile >> 2) > cur_w + 1) {               // only the K stream (one tile ahead) can get here
+                cur = nxt;
+                ++cur_w;
+                const int pi = (cur_w + 1) * 32 + lane;
+                nxt = pi < n_pages_item ? bt[pi] : 0;
+            }
+            const bool in_cur = (tile >> 2) == cur_w;                     // uniform
+            const int n_pages = min(8, n_pages_item - tile * 8);          // 1..8
+            const uint32_t slot = ld_cnt % kStages;
+            CP_PWAIT(1, &misc->kv_empty[slot], ((ld_cnt / kStages) & 1) ^ 1);
+            const bool leader = ptx::elect_one();
+            if (leader) ptx::mbar_arrive_expect_tx(&misc->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u);
+            uint8_t* dst = kv_base + slot * L::kSlotBytes;
+            // every operand below is warp-uniform (shuffle from a uniform lane), so the TMA issue
+            // needs no per-lane serialisation
 #pragma unroll
-            for (int h = 0; h < L::kHalves; ++h)
-                ptx::tma_load_3d(dst + h * L::kHalfBytes, tmap, &misc->kv_full[slot], h * 64, 0, slab);
+            for (int j = 0; j < 8; ++j) {
+                const int pg = __shfl_sync(0xffffffffu, in_cur ? cur : nxt, (tile & 3) * 8 + j);
+                if (j < n_pages) {
+                    const int slab = (pg * 2 + is_v) * p.sh.Hkv + kv_head;
+                    if (leader) ptx::tma_load_5d(dst + j * L::kPageBytes, tmap, &misc->kv_full[slot], 0, 0, 0, 0, slab);
+                }
+            }
+            __syncwarp();
+            ++ld_cnt;
         }
-        __syncwarp();
-        ++ld_cnt;
     }
 }
 
@@ -122,8 +187,10 @@ template <int D>
 __device__ __forceinline__ void tc_mma_item(const WorkItem& it, uint32_t smem_base, TcMisc* misc, uint32_t tmem,
                                             uint32_t& cons_cnt, uint32_t& gt, uint32_t item_cnt) {
     using L = TcLayout<D>;
-    const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
-    const bool swap = it.kind == kKindSwap;
+    // the whole warp runs this convergently with warp-uniform values; only the tcgen05 issue is
+    // elected, so descriptors stay in uniform registers
+    const int n_tiles = (__shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0) + kKeyTile - 1) / kKeyTile;
+    const bool swap = __shfl_sync(0xffffffffu, it.kind, 0) == kKindSwap;
     const uint32_t q_base = smem_base + L::kOffQ, p_base = smem_base + L::kOffP, kv_base = smem_base + L::kOffKV;
     // tile kind: S = Q K^T (M 128 rows, N 128 keys); O += P V (M 128, N D, V is MN-major B)
     // swap kind: S^T = K Q^T (M 128 keys, N 16);     O^T += V^T P^T (M 128 = D, N 16, V^T is MN-major A)
@@ -131,52 +198,58 @@ __device__ __forceinline__ void tc_mma_item(const WorkItem& it, uint32_t smem_ba
     const uint32_t idesc_pv = swap ? ptx::umma_idesc_bf16(128, 16, true, false) : ptx::umma_idesc_bf16(128, D, false, true);
     const uint32_t small_half = 2048;          // 16 rows x 128 B (Q^T / P^T halves in the swap kind)
 
-    ptx::mbar_wait(&misc->q_full, item_cnt & 1);
+    CP_PWAIT(2, &misc->q_full, item_cnt & 1);
     ptx::tc_fence_after();
 
     auto issue_qk = [&](uint32_t buf) {
         const uint32_t slot = cons_cnt % kStages;
-        ptx::mbar_wait(&misc->kv_full[slot], (cons_cnt / kStages) & 1);
+        CP_PWAIT(3, &misc->kv_full[slot], (cons_cnt / kStages) & 1);
         ptx::tc_fence_after();
         const uint32_t k_tile = kv_base + slot * L::kSlotBytes;
         const uint32_t d_tmem = tmem + (buf ? kColS1 : kColS0);
+        if (ptx::elect_one()) {
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
-            const uint32_t koff = (ks >> 2) * L::kHalfBytes + (ks & 3) * 32;
+            const uint32_t qoff_t = (ks >> 2) * L::kHalfBytes + (ks & 3) * 32;     // Q tile: halves 16 KB apart
+            const uint32_t koff = (ks >> 2) * 1024 + (ks & 3) * 32;                // K slot: halves 1 KB apart
+            const uint64_t k_desc = ptx::umma_desc_sw128(k_tile + koff, 16, L::kGroupBytes);
             if (!swap) {
-                ptx::umma_ss(d_tmem, ptx::umma_desc_sw128(q_base + koff, 16, 1024),
-                             ptx::umma_desc_sw128(k_tile + koff, 16, 1024), idesc_qk, ks > 0);
+                ptx::umma_ss(d_tmem, ptx::umma_desc_sw128(q_base + qoff_t, 16, 1024), k_desc, idesc_qk, ks > 0);
             } else {
                 const uint32_t qoff = (ks >> 2) * small_half + (ks & 3) * 32;
-                ptx::umma_ss(d_tmem, ptx::umma_desc_sw128(k_tile + koff, 16, 1024),
-                             ptx::umma_desc_sw128(q_base + qoff, 16, 1024), idesc_qk, ks > 0);
+                ptx::umma_ss(d_tmem, k_desc, ptx::umma_desc_sw128(q_base + qoff, 16, 1024), idesc_qk, ks > 0);
             }
         }
         ptx::umma_commit(&misc->kv_empty[slot]);
         ptx::umma_commit(&misc->s_full[buf]);
+        }
+        __syncwarp();
         ++cons_cnt;
     };
     auto issue_pv = [&](bool first) {
-        ptx::mbar_wait(&misc->p_full, gt & 1);
+        CP_PWAIT(4, &misc->p_full, gt & 1);
         const uint32_t slot = cons_cnt % kStages;
-        ptx::mbar_wait(&misc->kv_full[slot], (cons_cnt / kStages) & 1);
+        CP_PWAIT(5, &misc->kv_full[slot], (cons_cnt / kStages) & 1);
         ptx::tc_fence_after();
         const uint32_t v_tile = kv_base + slot * L::kSlotBytes;
         const uint32_t d_tmem = tmem + kColO;
+        if (ptx::elect_one()) {
 #pragma unroll
         for (int ks = 0; ks < kKeyTile / 16; ++ks) {
-            // V: 16 key rows (= MMA K) of 128 B per 64-wide half of D; halves are kHalfBytes apart (LBO)
-            const uint64_t v_desc = ptx::umma_desc_sw128(v_tile + ks * 2048, L::kHalfBytes, 1024);
+            // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
+            const uint64_t v_desc = ptx::umma_desc_sw128(v_tile + ks * L::kPageBytes, 1024, L::kGroupBytes);
             if (!swap) {
                 const uint32_t poff = (ks >> 2) * L::kHalfBytes + (ks & 3) * 32;
                 ptx::umma_ss(d_tmem, ptx::umma_desc_sw128(p_base + poff, 16, 1024), v_desc, idesc_pv, !first || ks > 0);
             } else {
-                const uint32_t poff = (ks >> 2) * small_half + (ks & 3) * 32;
+                const uint32_t poff = (gt & 1) * 4096 + (ks >> 2) * small_half + (ks & 3) * 32;   // P^T is double buffered
                 ptx::umma_ss(d_tmem, v_desc, ptx::umma_desc_sw128(p_base + poff, 16, 1024), idesc_pv, !first || ks > 0);
             }
         }
         ptx::umma_commit(&misc->kv_empty[slot]);
-        ptx::umma_commit(&misc->pv_done);
+        ptx::umma_commit(&misc->pv_done[gt & 1]);
+        }
+        __syncwarp();
         ++cons_cnt;
         ++gt;
     };
@@ -227,7 +300,7 @@ __device__ __forceinline__ void tc_softmax_tile(const WorkItem& it, const TcPara
     for (int k = 0; k < n_tiles; ++k) {
         const int ts = it.kv_begin + k * kKeyTile;
         const uint32_t buf = gt & 1;
-        ptx::mbar_wait(&misc->s_full[buf], (gt >> 1) & 1);
+        CP_PWAIT(6, &misc->s_full[buf], (gt >> 1) & 1);
         ptx::tc_fence_after();
         uint32_t sr[128];
 #pragma unroll
@@ -272,7 +345,7 @@ __device__ __forceinline__ void tc_softmax_tile(const WorkItem& it, const TcPara
         }
         l = l * alpha + sum;
         if (k > 0) {                                    // PV(k-1) done: P smem free, O readable
-            ptx::mbar_wait(&misc->pv_done, (gt - 1) & 1);
+            CP_PWAIT(7, &misc->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
             ptx::tc_fence_after();
         }
 #pragma unroll
@@ -298,7 +371,7 @@ __device__ __forceinline__ void tc_softmax_tile(const WorkItem& it, const TcPara
     }
 
     // ---- epilogue: O row from TMEM -> out (bf16, normalised) or split workspace (fp32, unnormalised)
-    ptx::mbar_wait(&misc->pv_done, (gt - 1) & 1);
+    CP_PWAIT(8, &misc->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
     ptx::tc_fence_after();
     const float inv = 1.f / l;
 #pragma unroll
@@ -327,24 +400,28 @@ __device__ __forceinline__ void tc_softmax_tile(const WorkItem& it, const TcPara
 }
 
 // ------------------------------------------------------------------------------------------
-// softmax warps, swap kind (D = 128, <= 16 rows): thread <-> key of the tile (S^T lane) during
-// the key loop, thread <-> d (O^T lane) for rescale / epilogue.  Column c = (token, head) row.
+// softmax warps, swap kind (D = 128, R <= RC <= 16 rows): thread <-> key of the tile (S^T lane)
+// during the key loop, thread <-> d (O^T lane) for rescale / epilogue.  Column c = (token, head)
+// row; columns in [R, RC) are computed as fully masked.  Straight-line code per column so the
+// independent chains interleave; the column max is one REDUX per column and warp.
 // ------------------------------------------------------------------------------------------
+template <int RC>
 __device__ __forceinline__ void tc_softmax_swap(const WorkItem& it, const TcParams& p, uint8_t* smem, TcMisc* misc,
                                                 uint32_t tmem, uint32_t& gt, int row, uint32_t lane_base, int swarp) {
     constexpr int D = 128;
     using L = TcLayout<D>;
     const Shape& sh = p.sh;
     const int G = sh.G;
-    const int R = it.q_tokens * G;                       // <= 16
+    const int R = it.q_tokens * G;                       // <= RC
     const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
     const int tok0 = p.meta.cu_q[it.req] + it.q_start;
     const int ctx = p.meta.ctx_off[it.req];
     const float scale = sh.sm_scale * 1.4426950408889634f;
     const int lane = row & 31;
+    CP_STAMP_INIT;
 
     // ---- Q^T -> smem: B operand [16 rows][D], K-major, 128B swizzle, halves 2 KB apart
-    for (int id = row; id < 16 * (D / 8); id += 128) {
+    for (int id = row; id < RC * (D / 8); id += 128) {
         const int r = id >> 4, c = id & 15;
         uint4 v = make_uint4(0, 0, 0, 0);
         if (r < R) {
@@ -355,11 +432,12 @@ __device__ __forceinline__ void tc_softmax_swap(const WorkItem& it, const TcPara
     }
     ptx::fence_proxy_async_smem();
     ptx::mbar_arrive(&misc->q_full);
+    CP_STAMP(10);
 
-    float m_ref[16], l_part[16];
-    int limit[16];
+    float m_ref[RC], l_part[RC];
+    int limit[RC];
 #pragma unroll
-    for (int c = 0; c < 16; ++c) {
+    for (int c = 0; c < RC; ++c) {
         m_ref[c] = -INFINITY;
         l_part[c] = 0.f;
         limit[c] = c < R ? min(it.kv_end, ctx + it.q_start + c / G + 1) : 0;
@@ -370,29 +448,33 @@ __device__ __forceinline__ void tc_softmax_swap(const WorkItem& it, const TcPara
     const int pchunk = (row & 63) >> 3;
 
     for (int k = 0; k < n_tiles; ++k) {
+        CP_STAMP(12);
         const int key = it.kv_begin + k * kKeyTile + row;
         const uint32_t buf = gt & 1;
-        ptx::mbar_wait(&misc->s_full[buf], (gt >> 1) & 1);
+        CP_PWAIT(6, &misc->s_full[buf], (gt >> 1) & 1);
         ptx::tc_fence_after();
-        uint32_t sr[16];
-        ptx::tmem_ld16(t_row + (buf ? kColS1 : kColS0), sr);
+        CP_STAMP(0);
+        uint32_t sr[RC];
+        ptx::tmem_ld<RC>(t_row + (buf ? kColS1 : kColS0), sr);
         ptx::tmem_wait_ld();
-        float sv[16];
+        CP_STAMP(1);
+        float sv[RC];
+        int* cm = reinterpret_cast<int*>(&misc->cmax[k & 1][swarp][0]);
 #pragma unroll
-        for (int c = 0; c < 16; ++c) {
+        for (int c = 0; c < RC; ++c) {
             sv[c] = key < limit[c] ? __uint_as_float(sr[c]) * scale : -INFINITY;
-            float w = sv[c];
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) w = fmaxf(w, __shfl_xor_sync(0xffffffffu, w, o));
-            if (lane == c) misc->cmax[k & 1][swarp][c] = w;       // lanes 0..15 publish one column each
+            const int w = __reduce_max_sync(0xffffffffu, ptx::f2ord(sv[c]));
+            if (lane == 0) cm[c] = w;
         }
+        CP_STAMP(2);
         ptx::named_bar_sync(1, 128);
+        CP_STAMP(3);
         bool any_rescale = false;
-        float alpha[16];
+        float alpha[RC];
+        const int* cm0 = reinterpret_cast<const int*>(&misc->cmax[k & 1][0][0]);
 #pragma unroll
-        for (int c = 0; c < 16; ++c) {
-            const float m_t = fmaxf(fmaxf(misc->cmax[k & 1][0][c], misc->cmax[k & 1][1][c]),
-                                    fmaxf(misc->cmax[k & 1][2][c], misc->cmax[k & 1][3][c]));
+        for (int c = 0; c < RC; ++c) {
+            const float m_t = ptx::ord2f(max(max(cm0[c], cm0[16 + c]), max(cm0[32 + c], cm0[48 + c])));
             alpha[c] = 1.f;
             if (m_t > m_ref[c] + kRescaleThreshold) {
                 alpha[c] = (m_ref[c] == -INFINITY) ? 0.f : ptx::ex2(m_ref[c] - m_t);
@@ -403,45 +485,55 @@ __device__ __forceinline__ void tc_softmax_swap(const WorkItem& it, const TcPara
             l_part[c] = l_part[c] * alpha[c] + pc;
             sv[c] = pc;
         }
-        if (k > 0) {
-            ptx::mbar_wait(&misc->pv_done, (gt - 1) & 1);
-            ptx::tc_fence_after();
+        CP_STAMP(4);
+        if (k >= 2) {                                    // PV(gt-2) done: this P^T buffer is free again
+            CP_PWAIT(7, &misc->pv_done[gt & 1], ((gt - 2) >> 1) & 1);
         }
+        {
+            uint8_t* ptb = pt + (gt & 1) * 4096;
 #pragma unroll
-        for (int c = 0; c < 16; ++c)
-            *reinterpret_cast<__nv_bfloat16*>(pt + c * 128 + ((pchunk ^ (c & 7)) << 4)) = __float2bfloat16_rn(sv[c]);
+            for (int c = 0; c < RC; ++c)
+                *reinterpret_cast<__nv_bfloat16*>(ptb + c * 128 + ((pchunk ^ (c & 7)) << 4)) = __float2bfloat16_rn(sv[c]);
+        }
+        CP_STAMP(5);
         if (k > 0 && any_rescale) {                      // uniform over the 128 threads
-            uint32_t o[16];
-            ptx::tmem_ld16(t_row + kColO, o);
+            CP_PWAIT(9, &misc->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
+            ptx::tc_fence_after();
+            uint32_t o[RC];
+            ptx::tmem_ld<RC>(t_row + kColO, o);
             ptx::tmem_wait_ld();
 #pragma unroll
-            for (int c = 0; c < 16; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha[c]);
-            ptx::tmem_st16(t_row + kColO, o);
+            for (int c = 0; c < RC; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha[c]);
+            ptx::tmem_st<RC>(t_row + kColO, o);
             ptx::tmem_wait_st();
         }
+        CP_STAMP(6);
         ptx::fence_proxy_async_smem();
+        CP_STAMP(7);
         ptx::tc_fence_before();
         ptx::mbar_arrive(&misc->p_full);
+        CP_STAMP(8);
         ++gt;
     }
+    CP_STAMP(12);
 
     // ---- column sums over the 128 key lanes
 #pragma unroll
-    for (int c = 0; c < 16; ++c) {
+    for (int c = 0; c < RC; ++c) {
         float w = l_part[c];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
-        if (lane == c) misc->lsum[swarp][c] = w;
+        if (lane == 0) misc->lsum[swarp][c] = w;
     }
     ptx::named_bar_sync(1, 128);
     // ---- epilogue: O^T[d = row][c] -> out / workspace
-    ptx::mbar_wait(&misc->pv_done, (gt - 1) & 1);
+    CP_PWAIT(8, &misc->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
     ptx::tc_fence_after();
-    uint32_t o[16];
-    ptx::tmem_ld16(t_row + kColO, o);
+    uint32_t o[RC];
+    ptx::tmem_ld<RC>(t_row + kColO, o);
     ptx::tmem_wait_ld();
 #pragma unroll
-    for (int c = 0; c < 16; ++c) {
+    for (int c = 0; c < RC; ++c) {
         if (c < R) {
             const float lc = misc->lsum[0][c] + misc->lsum[1][c] + misc->lsum[2][c] + misc->lsum[3][c];
             if (it.partial_row < 0) {
@@ -455,6 +547,7 @@ __device__ __forceinline__ void tc_softmax_swap(const WorkItem& it, const TcPara
     }
     ptx::tc_fence_before();
     ptx::named_bar_sync(1, 128);                         // lsum / cmax are reused by the next item
+    CP_STAMP(9);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -475,10 +568,16 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tmap) {
         ptx::mbar_init(&misc->s_full[0], 1);
         ptx::mbar_init(&misc->s_full[1], 1);
         ptx::mbar_init(&misc->p_full, 128);
-        ptx::mbar_init(&misc->pv_done, 1);
+        ptx::mbar_init(&misc->pv_done[0], 1);
+        ptx::mbar_init(&misc->pv_done[1], 1);
+        for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&misc->item_full[i], 1); ptx::mbar_init(&misc->item_empty[i], 129); }
         ptx::fence_barrier_init();
         ptx::prefetch_tmap(&tmap);
     }
+#if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
+    if (threadIdx.x < 16) misc->prof[threadIdx.x] = 0;
+    const long long t_start__ = clock64();
+#endif
     if (warp == 1) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
     // stale shared memory may hold NaN bit patterns; tiles are only partly overwritten by short
     // requests, and 0 x NaN would poison the accumulators
@@ -490,33 +589,53 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tmap) {
     ptx::tc_fence_after();
     const uint32_t tmem = misc->tmem_base;
 
-    uint32_t ld_cnt = 0, cons_cnt = 0, gt = 0, item_cnt = 0;
-    while (true) {
-        if (threadIdx.x == 0) misc->item = atomicAdd(&p.counters[0], 1);
-        __syncthreads();
-        const int item = misc->item;
-        if (item >= p.meta.n_work) break;
-        const WorkItem it = p.meta.work[item];
-        if (warp == 0) {
-            tc_produce_item<D>(it, p.meta, p.sh, &tmap, smem + L::kOffKV, misc, ld_cnt, lane);
-        } else if (warp == 1) {
-            if (lane == 0) tc_mma_item<D>(it, ptx::smem_u32(smem), misc, tmem, cons_cnt, gt, item_cnt);
+    // Roles run decoupled: the producer publishes items through misc->items[]; each consumer copies
+    // the item, frees the ring slot at once, and works from its private copy.
+    if (warp == 0) {
+        tc_producer<D>(p, &tmap, smem + L::kOffKV, misc, lane);
+    } else if (warp == 1) {
+        uint32_t cons_cnt = 0, gt = 0, item_cnt = 0;
+        for (;;) {
+            const uint32_t islot = item_cnt % kItemRing;
+            CP_PWAIT(10, &misc->item_full[islot], (item_cnt / kItemRing) & 1);
+            const WorkItem it = misc->items[islot];
             __syncwarp();
-        } else {
-            const uint32_t lane_base = (warp & 3) * 32;
-            const int row = lane_base + lane;
+            if (lane == 0) ptx::mbar_arrive(&misc->item_empty[islot]);
+            if (it.kind < 0) break;
+            tc_mma_item<D>(it, ptx::smem_u32(smem), misc, tmem, cons_cnt, gt, item_cnt);
+            ++item_cnt;
+        }
+    } else {
+        const uint32_t lane_base = (warp & 3) * 32;
+        const int row = lane_base + lane;
+        uint32_t gt = 0, item_cnt = 0;
+        for (;;) {
+            const uint32_t islot = item_cnt % kItemRing;
+            CP_PWAIT(11, &misc->item_full[islot], (item_cnt / kItemRing) & 1);
+            const WorkItem it = misc->items[islot];
+            ptx::mbar_arrive(&misc->item_empty[islot]);
+            if (it.kind < 0) break;
             if (it.kind == kKindSwap) {
-                if constexpr (D == 128) tc_softmax_swap(it, p, smem, misc, tmem, gt, row, lane_base, warp & 3);
+                if constexpr (D == 128) {
+                    const int R = it.q_tokens * p.sh.G;
+                    if (R <= 4) tc_softmax_swap<4>(it, p, smem, misc, tmem, gt, row, lane_base, warp & 3);
+                    else if (R <= 8) tc_softmax_swap<8>(it, p, smem, misc, tmem, gt, row, lane_base, warp & 3);
+                    else tc_softmax_swap<16>(it, p, smem, misc, tmem, gt, row, lane_base, warp & 3);
+                }
             } else {
                 tc_softmax_tile<D>(it, p, smem, misc, tmem, gt, row, lane_base);
             }
+            ++item_cnt;
         }
-        ++item_cnt;
-        __syncthreads();
     }
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 1) ptx::tmem_dealloc(tmem, kTmemCols);
+#if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
+    if (threadIdx.x == 0) misc->prof[15] = (unsigned long long)(clock64() - t_start__);
+    __syncthreads();
+    if (threadIdx.x < 16 && p.prof) p.prof[blockIdx.x * 16 + threadIdx.x] = misc->prof[threadIdx.x];
+#endif
     if (threadIdx.x == 0) {
         __threadfence();
         if (atomicAdd(&p.counters[1], 1) == (int)gridDim.x - 1) {      // last CTA re-arms the counters
