@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -430,7 +431,8 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
     }
     if (m.n_work > 0) {
         TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
-        const int grid = std::min(c->n_sm, m.n_work);
+        int grid = std::min(c->n_sm, m.n_work);
+        if (const char* e = getenv("CP_TC_GRID")) grid = std::max(1, std::min(grid, atoi(e)));   // experiments only
         attn_tc_kernel<D><<<grid, kTcThreads, TcLayout<D>::kTotal, stream>>>(p, *tmap);
         CP_CUDA(cudaGetLastError());
         ++*launches;

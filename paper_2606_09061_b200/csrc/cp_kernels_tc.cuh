@@ -28,7 +28,8 @@
 
 namespace cp {
 
-constexpr int kTcThreads = 192;
+constexpr int kProducers = 2;                // TMA producer warps (issue rate scales with warps)
+constexpr int kTcThreads = 32 * (kProducers + 5);   // producers, MMA issuer, 4 softmax warps
 constexpr int kStages = 5;
 constexpr int kTmemCols = 512;
 constexpr int kItemRing = 2;
@@ -55,7 +56,7 @@ struct TcLayout {
 
 // Optional role-level wait-time profile (build with -DCP_TC_PROF; debugging aid only).
 #ifdef CP_TC_PROF2
-#define CP_STAMP(id) do { if (threadIdx.x == 128) { long long t__ = clock64(); misc->prof[id] += (unsigned long long)(t__ - tprev__); tprev__ = t__; } } while (0)
+#define CP_STAMP(id) do { if (threadIdx.x == 32 * (kProducers + 2)) { long long t__ = clock64(); misc->prof[id] += (unsigned long long)(t__ - tprev__); tprev__ = t__; } } while (0)
 #define CP_STAMP_INIT long long tprev__ = clock64()
 #else
 #define CP_STAMP(id) do {} while (0)
@@ -66,7 +67,7 @@ struct TcLayout {
     do {                                                                              \
         const long long t0__ = clock64();                                             \
         ptx::mbar_wait(bar, par);                                                     \
-        if ((threadIdx.x & 31) == 0 && (threadIdx.x < 64 || threadIdx.x == 128))      \
+        if (threadIdx.x == 0 || threadIdx.x == 32 * kProducers || threadIdx.x == 32 * (kProducers + 2)) \
             misc->prof[id] += (unsigned long long)(clock64() - t0__);                 \
     } while (0)
 #else
@@ -117,50 +118,58 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 // ------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void tc_producer(const TcParams& p, const CUtensorMap* tmap, uint8_t* kv_base,
-                                            TcMisc* misc, int lane) {
+                                            TcMisc* misc, int lane, int pw) {
     using L = TcLayout<D>;
-    uint32_t ld_cnt = 0, item_cnt = 0;
+    uint32_t ld_base = 0, item_cnt = 0;          // ld_base: tile loads of all previous items
     for (;;) {
-        int idx = 0;
-        if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
-        idx = __shfl_sync(0xffffffffu, idx, 0);
-        const bool done = idx >= p.meta.n_work;
-        // one int32 of the 32-byte WorkItem per lane 0..7
-        int w = 0;
-        if (!done && lane < 8) w = reinterpret_cast<const int32_t*>(p.meta.work + idx)[lane];
-        if (done && lane == 7) w = -1;                                   // kind = -1: sentinel
         const uint32_t islot = item_cnt % kItemRing;
-        CP_PWAIT(0, &misc->item_empty[islot], ((item_cnt / kItemRing) & 1) ^ 1);
-        if (lane < 8) reinterpret_cast<int32_t*>(&misc->items[islot])[lane] = w;
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&misc->item_full[islot]);
+        int w;
+        if (pw == 0) {                           // producer 0 fetches the next item and publishes it
+            int idx = 0;
+            if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
+            idx = __shfl_sync(0xffffffffu, idx, 0);
+            const bool done = idx >= p.meta.n_work;
+            w = 0;                               // one int32 of the 32-byte WorkItem per lane 0..7
+            if (!done && lane < 8) w = reinterpret_cast<const int32_t*>(p.meta.work + idx)[lane];
+            if (done && lane == 7) w = -1;       // kind = -1: sentinel
+            CP_PWAIT(0, &misc->item_empty[islot], ((item_cnt / kItemRing) & 1) ^ 1);
+            if (lane < 8) reinterpret_cast<int32_t*>(&misc->items[islot])[lane] = w;
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&misc->item_full[islot]);
+        } else {
+            CP_PWAIT(0, &misc->item_full[islot], (item_cnt / kItemRing) & 1);
+            w = lane < 8 ? reinterpret_cast<const int32_t*>(&misc->items[islot])[lane] : 0;
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&misc->item_empty[islot]);
+        }
         ++item_cnt;
-        if (done) break;
+        if (__shfl_sync(0xffffffffu, w, 7) < 0) break;
         const int req = __shfl_sync(0xffffffffu, w, 0), kv_head = __shfl_sync(0xffffffffu, w, 1);
         const int kv_begin = __shfl_sync(0xffffffffu, w, 4), kv_end = __shfl_sync(0xffffffffu, w, 5);
         const int n_tiles = (kv_end - kv_begin + kKeyTile - 1) / kKeyTile;
         const int32_t* bt = p.meta.block_table + p.meta.bt_off[req] + (kv_begin >> 4);
         const int n_pages_item = (kv_end - kv_begin + 15) >> 4;
-        // page-id windows of 32 pages (4 tiles): cur = window cur_w, nxt = window cur_w + 1
+        // page-id windows of 32 pages (4 tiles), one id per lane: cur = window cur_w, nxt = the next.
+        // This warp's tile sequence is monotone, so windows only ever advance.
         int cur_w = 0;
         int cur = lane < n_pages_item ? bt[lane] : 0;
         int nxt = 32 + lane < n_pages_item ? bt[32 + lane] : 0;
-        for (int i = 0; i < 2 * n_tiles; ++i) {
+        for (int i = pw; i < 2 * n_tiles; i += kProducers) {
             int is_v, tile;
             if (i == 0) { is_v = 0; tile = 0; }
             else if (i == 2 * n_tiles - 1) { is_v = 1; tile = n_tiles - 1; }
             else if (i & 1) { is_v = 0; tile = (i + 1) >> 1; }
             else { is_v = 1; tile = (i >> 1) - 1; }
-            if ((tile >> 2) > cur_w + 1) {               // only the K stream (one tile ahead) can get here
+            while ((tile >> 2) > cur_w) {
                 cur = nxt;
                 ++cur_w;
                 const int pi = (cur_w + 1) * 32 + lane;
                 nxt = pi < n_pages_item ? bt[pi] : 0;
             }
-            const bool in_cur = (tile >> 2) == cur_w;                     // uniform
             const int n_pages = min(8, n_pages_item - tile * 8);          // 1..8
-            const uint32_t slot = ld_cnt % kStages;
-            CP_PWAIT(1, &misc->kv_empty[slot], ((ld_cnt / kStages) & 1) ^ 1);
+            const uint32_t ld = ld_base + i;
+            const uint32_t slot = ld % kStages;
+            CP_PWAIT(1, &misc->kv_empty[slot], ((ld / kStages) & 1) ^ 1);
             const bool leader = ptx::elect_one();
             if (leader) ptx::mbar_arrive_expect_tx(&misc->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u);
             uint8_t* dst = kv_base + slot * L::kSlotBytes;
@@ -168,15 +177,15 @@ __device__ __forceinline__ void tc_producer(const TcParams& p, const CUtensorMap
             // needs no per-lane serialisation
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                const int pg = __shfl_sync(0xffffffffu, in_cur ? cur : nxt, (tile & 3) * 8 + j);
+                const int pg = __shfl_sync(0xffffffffu, cur, (tile & 3) * 8 + j);
                 if (j < n_pages) {
                     const int slab = (pg * 2 + is_v) * p.sh.Hkv + kv_head;
                     if (leader) ptx::tma_load_5d(dst + j * L::kPageBytes, tmap, &misc->kv_full[slot], 0, 0, 0, 0, slab);
                 }
             }
             __syncwarp();
-            ++ld_cnt;
         }
+        ld_base += 2 * n_tiles;
     }
 }
 
@@ -570,7 +579,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tmap) {
         ptx::mbar_init(&misc->p_full, 128);
         ptx::mbar_init(&misc->pv_done[0], 1);
         ptx::mbar_init(&misc->pv_done[1], 1);
-        for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&misc->item_full[i], 1); ptx::mbar_init(&misc->item_empty[i], 129); }
+        for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&misc->item_full[i], 1); ptx::mbar_init(&misc->item_empty[i], 128 + kProducers); }
         ptx::fence_barrier_init();
         ptx::prefetch_tmap(&tmap);
     }
@@ -578,7 +587,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tmap) {
     if (threadIdx.x < 16) misc->prof[threadIdx.x] = 0;
     const long long t_start__ = clock64();
 #endif
-    if (warp == 1) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
+    if (warp == kProducers) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
     // stale shared memory may hold NaN bit patterns; tiles are only partly overwritten by short
     // requests, and 0 x NaN would poison the accumulators
     for (uint32_t i = threadIdx.x * 16; i < L::kOffMisc; i += kTcThreads * 16)
@@ -591,9 +600,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tmap) {
 
     // Roles run decoupled: the producer publishes items through misc->items[]; each consumer copies
     // the item, frees the ring slot at once, and works from its private copy.
-    if (warp == 0) {
-        tc_producer<D>(p, &tmap, smem + L::kOffKV, misc, lane);
-    } else if (warp == 1) {
+    if (warp < kProducers) {
+        tc_producer<D>(p, &tmap, smem + L::kOffKV, misc, lane, warp);
+    } else if (warp == kProducers) {
         uint32_t cons_cnt = 0, gt = 0, item_cnt = 0;
         for (;;) {
             const uint32_t islot = item_cnt % kItemRing;
@@ -630,7 +639,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tmap) {
     }
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 1) ptx::tmem_dealloc(tmem, kTmemCols);
+    if (warp == kProducers) ptx::tmem_dealloc(tmem, kTmemCols);
 #if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
     if (threadIdx.x == 0) misc->prof[15] = (unsigned long long)(clock64() - t_start__);
     __syncthreads();
