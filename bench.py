@@ -101,8 +101,12 @@ def oracle_sample_rate(spec, q_bits, cache_bits, target_s, seed=0):
     keys_of_tok = spec.ctx_off[tok_req].astype(np.int64) + (np.arange(spec.T) - cu[tok_req]) + 1
 
     def run(n):
-        tok = rng.integers(0, spec.T, size=n).astype(np.int64)
-        head = rng.integers(0, spec.Hq, size=n).astype(np.int32)
+        if n >= spec.T * spec.Hq:                          # the whole batch fits the time budget
+            tok = np.repeat(np.arange(spec.T, dtype=np.int64), spec.Hq)
+            head = np.tile(np.arange(spec.Hq, dtype=np.int32), spec.T)
+        else:
+            tok = rng.integers(0, spec.T, size=n).astype(np.int64)
+            head = rng.integers(0, spec.Hq, size=n).astype(np.int32)
         t0 = time.perf_counter()
         ora.attention(q_bits, cache_bits, spec.q_len, spec.ctx_off, tabs, spec.sm_scale, rows=(tok, head))
         return time.perf_counter() - t0, int(keys_of_tok[tok].sum())
@@ -113,13 +117,31 @@ def oracle_sample_rate(spec, q_bits, cache_bits, target_s, seed=0):
     dt, pairs = run(n)
     total_pairs = spec.causal_pairs() * spec.Hq
     full_s = dt * total_pairs / max(pairs, 1)
+    n = min(n, spec.T * spec.Hq)
     desc = (f"{n} seeded (token,head) rows of {spec.T * spec.Hq} ({pairs} of {total_pairs} causal "
-            f"pairs) in {dt:.2f} s; full-batch time extrapolated by the causal-pair ratio")
+            f"pairs) in {dt:.2f} s" + ("; the whole batch" if n == spec.T * spec.Hq else
+                                       "; full-batch time extrapolated by the causal-pair ratio"))
     return spec.T / full_s, threads, desc
 
 
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def max_over_ranks(ms: float, device="cpu") -> float:
+    """Device time of the slowest replica (the contract's max-over-ranks); identity at N = 1."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank_step: int, steps: int, world: int, ms_max: float) -> float:
+    """Replicas only, weak scaling: every rank processes the same number of units per step."""
+    return world * units_per_rank_step * steps / (ms_max * 1e-3)
 
 
 def run_ours(args):
@@ -170,10 +192,7 @@ def run_ours(args):
     barrier()
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dev)
     rows = ctx.cp_latency_table()
     step_us = np.array([r.us for r in rows], dtype=np.float64)
     info = ctx.cp_get_batch_info()
@@ -198,10 +217,7 @@ def run_ours(args):
     e1.record()
     barrier()
     e2e_ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, dev)
     ctx.cp_latency_table()
     meta_bytes = 4 * (4 * spec.n_reqs + 2 + n_pages + spec.T) + 32 * (info.n_work_items + info.n_combine_items)
     h2d = int(hq.numel() * 2 + hk.numel() * 2 + hv_.numel() * 2 + meta_bytes)
@@ -212,7 +228,7 @@ def run_ours(args):
         return
     peaks = measured_peaks()
     ms_per_step = ms_total / args.steps
-    tokens_per_s = world * spec.T * args.steps / (ms_total * 1e-3)
+    tokens_per_s = whole_job_rate(spec.T, args.steps, world, ms_total)
     # roofline for the step's kernels (append + attention + combine), CUDA events on the launch stream
     attn_us = float(np.mean(step_us)) if len(step_us) else ms_per_step * 1e3
     bytes_alg, flops_alg = spec.algorithmic_bytes(), spec.flops()
@@ -235,7 +251,7 @@ def run_ours(args):
                    "parallelism": "replicas" if world > 1 else "single", "kernel_variant": args.variant,
                    "work_items": info.n_work_items, "combine_items": info.n_combine_items},
         "clocks": clocks,
-        "e2e": {"value": world * spec.T * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+        "e2e": {"value": whole_job_rate(spec.T, args.steps, world, e2e_ms), "unit": UNIT,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps},
         "gpu_launches": int(info.kernels_per_step * args.steps),
         "iteration_us": {"step_incl_build_batch": ms_per_step * 1e3, "attention_step_mean": attn_us,
