@@ -371,7 +371,7 @@ static int launch_simt(cp_ctx* c, const __nv_bfloat16* q, const __nv_bfloat16* c
         CP_CUDA(cudaGetLastError());
     }
     if (m.n_combine > 0) {
-        combine_kernel<D><<<m.n_combine, 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
+        combine_kernel<D><<<dim3(m.n_combine, 32), 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
         CP_CUDA(cudaGetLastError());
     }
     return CP_OK;
@@ -439,7 +439,7 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
         c->info.grid_attn = grid;
     }
     if (m.n_combine > 0) {
-        combine_kernel<D><<<m.n_combine, 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
+        combine_kernel<D><<<dim3(m.n_combine, 32), 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
         CP_CUDA(cudaGetLastError());
         ++*launches;
     }

@@ -125,7 +125,10 @@ attn_simt_kernel(BatchMeta meta, Shape sh, const __nv_bfloat16* __restrict__ q,
 }
 
 // ---------------------------------------------------------------------------------
-// H5: out = sum_s w_s O_s / sum_s w_s l_s, w_s = 2^(m_s - max m).  Warp per row.
+// H5: out = sum_s w_s O_s / sum_s w_s l_s, w_s = 2^(m_s - max m).  One warp per row:
+// grid (n_combine, ceil(128 / 4)), warp w of block (i, y) merges row 4y + w of item i.  The
+// (m, l) pairs of up to 32 splits are read one per lane and the weights broadcast by shuffle, so
+// the O_s loads of a row are independent and issue back to back.
 // ---------------------------------------------------------------------------------
 template <int D>
 __global__ void __launch_bounds__(128)
@@ -133,33 +136,55 @@ combine_kernel(BatchMeta meta, Shape sh, const float* __restrict__ part_o,
                const float2* __restrict__ part_ml, __nv_bfloat16* __restrict__ out) {
     constexpr int EPL = D / 32;
     const CombineItem it = meta.combine[blockIdx.x];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int R = it.q_tokens * sh.G;
-    for (int r = warp; r < R; r += nwarps) {
-        float M = -INFINITY;
-        for (int s = 0; s < it.n_splits; ++s)
-            M = fmaxf(M, part_ml[(int64_t)it.partial_row + (int64_t)s * R + r].x);
-        float L = 0.f, acc[EPL];
+    const int r = blockIdx.y * 4 + warp;
+    if (r >= R) return;
+    const int64_t base = (int64_t)it.partial_row + r;
+    float M = -INFINITY;
+    for (int s0 = 0; s0 < it.n_splits; s0 += 32) {
+        const int s = s0 + lane;
+        float m = s < it.n_splits ? part_ml[base + (int64_t)s * R].x : -INFINITY;
 #pragma unroll
-        for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
-        for (int s = 0; s < it.n_splits; ++s) {
-            const int64_t pr = (int64_t)it.partial_row + (int64_t)s * R + r;
-            const float2 ml = part_ml[pr];
-            const float w = exp2f(ml.x - M);               // empty split: m = -inf -> w = 0
-            L += w * ml.y;
-            const float* po = part_o + pr * D + lane * EPL;
-#pragma unroll
-            for (int e = 0; e < EPL; ++e) acc[e] += w * po[e];
-        }
-        const int tok = it.tok0 + r / sh.G;
-        const int h = it.kv_head * sh.G + r % sh.G;
-        const float inv = 1.f / L;
-        __nv_bfloat16* op = out + ((int64_t)tok * sh.Hq + h) * D + lane * EPL;
-#pragma unroll
-        for (int e = 0; e < EPL; e += 2)
-            *reinterpret_cast<__nv_bfloat162*>(op + e) =
-                __floats2bfloat162_rn(acc[e] * inv, acc[e + 1] * inv);
+        for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        M = fmaxf(M, m);
     }
+    float L = 0.f, acc[EPL];
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+    for (int s0 = 0; s0 < it.n_splits; s0 += 32) {
+        const int s = s0 + lane;
+        float w = 0.f, wl = 0.f;
+        if (s < it.n_splits) {
+            const float2 ml = part_ml[base + (int64_t)s * R];
+            w = (ml.x == -INFINITY) ? 0.f : exp2f(ml.x - M);      // empty split: m = -inf -> w = 0
+            wl = w * ml.y;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) wl += __shfl_xor_sync(0xffffffffu, wl, o);
+        L += wl;
+        const int ns = min(32, it.n_splits - s0);
+#pragma unroll 4
+        for (int j = 0; j < ns; ++j) {
+            const float wj = __shfl_sync(0xffffffffu, w, j);
+            const float* po = part_o + (base + (int64_t)(s0 + j) * R) * D + lane * EPL;
+            if constexpr (EPL == 4) {
+                const float4 v = *reinterpret_cast<const float4*>(po);
+                acc[0] += wj * v.x; acc[1] += wj * v.y; acc[2] += wj * v.z; acc[3] += wj * v.w;
+            } else {
+                const float2 v = *reinterpret_cast<const float2*>(po);
+                acc[0] += wj * v.x; acc[1] += wj * v.y;
+            }
+        }
+    }
+    const int tok = it.tok0 + r / sh.G;
+    const int h = it.kv_head * sh.G + r % sh.G;
+    const float inv = 1.f / L;
+    __nv_bfloat16* op = out + ((int64_t)tok * sh.Hq + h) * D + lane * EPL;
+#pragma unroll
+    for (int e = 0; e < EPL; e += 2)
+        *reinterpret_cast<__nv_bfloat162*>(op + e) =
+            __floats2bfloat162_rn(acc[e] * inv, acc[e + 1] * inv);
 }
 
 }  // namespace cp

@@ -112,7 +112,8 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 // ------------------------------------------------------------------------------------------
 // producer warp: fetches work items (atomic counter), publishes them to the other roles through
 // a small smem ring, and streams the K and V tiles of each item into the slot ring in
-// consumption order  K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1).  It runs ahead of the
+// consumption order  K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1)  (tile kind) or
+// K0, V0, K1, V1, ... (swap kind).  It runs ahead of the
 // consumers by up to kStages tile loads, across item boundaries.  Page ids are prefetched 32 at
 // a time (one per lane) so no dependent global load sits between two TMA issues.
 // ------------------------------------------------------------------------------------------
@@ -154,9 +155,11 @@ __device__ __forceinline__ void tc_producer(const TcParams& p, const CUtensorMap
         int cur_w = 0;
         int cur = lane < n_pages_item ? bt[lane] : 0;
         int nxt = 32 + lane < n_pages_item ? bt[32 + lane] : 0;
+        const bool swap = __shfl_sync(0xffffffffu, w, 7) == kKindSwap;
         for (int i = pw; i < 2 * n_tiles; i += kProducers) {
             int is_v, tile;
-            if (i == 0) { is_v = 0; tile = 0; }
+            if (swap) { is_v = i & 1; tile = i >> 1; }                   // K0, V0, K1, V1, ...
+            else if (i == 0) { is_v = 0; tile = 0; }
             else if (i == 2 * n_tiles - 1) { is_v = 1; tile = n_tiles - 1; }
             else if (i & 1) { is_v = 0; tile = (i + 1) >> 1; }
             else { is_v = 1; tile = (i >> 1) - 1; }
@@ -263,10 +266,21 @@ __device__ __forceinline__ void tc_mma_item(const WorkItem& it, uint32_t smem_ba
         ++gt;
     };
 
-    issue_qk(gt & 1);
-    for (int k = 0; k < n_tiles; ++k) {
-        if (k + 1 < n_tiles) issue_qk((gt + 1) & 1);
-        issue_pv(k == 0);
+    if (swap) {
+        // QK(k+1) is issued only after p_full(k) was observed: the swap-kind softmax has no other
+        // back-pressure (P^T is double buffered), and without it a fast softmax could complete
+        // p_full phase k+1 before this thread looked at phase k (parity aliasing -> deadlock).
+        // The step is HBM-bound; the lost QK/softmax overlap is not on the critical path.
+        for (int k = 0; k < n_tiles; ++k) {
+            issue_qk(gt & 1);
+            issue_pv(k == 0);
+        }
+    } else {
+        issue_qk(gt & 1);
+        for (int k = 0; k < n_tiles; ++k) {
+            if (k + 1 < n_tiles) issue_qk((gt + 1) & 1);
+            issue_pv(k == 0);
+        }
     }
 }
 

@@ -161,3 +161,33 @@ def test_latency_table_rows():
     assert (r.n_prefill, r.n_decode, r.iter) == (2, 2, 0)
     assert ctx.cp_latency_table() == []
     ctx.close()
+
+
+def test_stress_long_decodes_with_chunk_no_deadlock():
+    """Regression: swap-kind (decode) items used to let the softmax warps run a full p_full phase
+    ahead of the MMA issuer (mbarrier parity aliasing -> rare deadlock, seen in the trace run).
+    Many back-to-back launches of the batch shape that triggered it; result checked on a sample."""
+    import torch
+    rng = np.random.default_rng(7)
+    ctx_dec = rng.integers(17000, 23500, size=13)
+    spec = wl.make_spec("stress", 32, 8, 128, 16, 24000, [1] * 13 + [1, 530],
+                        list(ctx_dec - 1) + [1992, 1500], seed=7)
+    dev = torch.device("cuda:0")
+    q, k_new, v_new, pool, compact = wl.device_values(spec, dev)
+    ctx = gu.make_ctx(spec, 0)
+    out = torch.empty((spec.T, spec.Hq, spec.D), device=dev, dtype=torch.bfloat16)
+    ctx.cp_build_batch(spec.q_len, spec.ctx_off, spec.block_tables)
+    for i in range(1500):
+        ctx.cp_attention_step(0, q, k_new if i == 0 else None, v_new if i == 0 else None, pool, out)
+        if i % 500 == 499:
+            torch.cuda.synchronize()
+            ctx.cp_latency_table()
+    torch.cuda.synchronize()
+    cache = gu.to_bits(compact)
+    tabs = spec.compact_tables()
+    ora.kv_append(gu.to_bits(k_new), gu.to_bits(v_new), cache, spec.q_len, spec.ctx_off, tabs)
+    tok, head = gu.sample_rows(spec, 96)
+    want = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale, rows=(tok, head))
+    got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)[tok, head]
+    gu.assert_close(got, want, "stress")
+    ctx.close()
