@@ -63,8 +63,10 @@ typedef struct {
     int64_t max_partial_rows; /* split-KV workspace rows ((D+2) fp32 each);
                                  0 = default 4 * max_tokens * Hq                  */
     int32_t device;           /* CUDA device ordinal                              */
-    int32_t kernel_variant;   /* 0 = default (tensor-core path where built),
-                                 1 = force the SIMT reference kernels (debug)     */
+    int32_t kernel_variant;   /* 0 = default: dual-lane tcgen05 kernel (chunk tiles and
+                                     decode streams co-resident on every SM),
+                                 1 = SIMT reference kernels (debug cross-check),
+                                 2 = single-lane tcgen05 kernel (round-1 baseline)   */
 } cp_config;
 
 /* One request of the iteration.  HOST pointers. */

@@ -13,6 +13,7 @@
 #include "cp_internal.h"
 #include "cp_kernels_simt.cuh"
 #ifdef CP_WITH_TC
+#include "cp_kernels_dl.cuh"
 #include "cp_kernels_tc.cuh"
 #endif
 
@@ -45,7 +46,8 @@ struct cp_ctx {
     Shape shape{};
     int n_sm = 148;
     int tq = 32;                       // tokens per Q tile = 128 / G
-    bool use_tc = false;
+    bool use_tc = false;               // a tensor-core variant (0 or 2)
+    bool use_dl = false;               // variant 0: the dual-lane kernel
 
     // limits
     size_t max_items = 0, max_combine = 0, meta_cap = 0;
@@ -79,7 +81,7 @@ struct cp_ctx {
     // host scratch reused across build_batch calls (no allocation in steady state)
     std::vector<WorkItem> items, sorted;
     std::vector<CombineItem> combines;
-    std::vector<int32_t> bucket;
+    std::vector<int32_t> bucket, plan, plan_prow;
 
     // tensor-core path: one TMA descriptor per KV pool pointer (one per layer), encoded once
     std::vector<std::pair<const void*, CUtensorMap>> tmaps;
@@ -107,14 +109,16 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     cudaDeviceProp prop{};
     if (cudaGetDeviceProperties(&prop, cfg->device) == cudaSuccess) c->n_sm = prop.multiProcessorCount;
 #ifdef CP_WITH_TC
-    c->use_tc = (cfg->kernel_variant == 0) && prop.major == 10;
+    c->use_tc = (cfg->kernel_variant == 0 || cfg->kernel_variant == 2) && prop.major == 10;
+    c->use_dl = c->use_tc && cfg->kernel_variant == 0;
 #endif
-    if (cfg->kernel_variant == 0 && !c->use_tc) {
+    if (cfg->kernel_variant < 0 || cfg->kernel_variant > 2) { delete c; cp_set_error("cp_create: kernel_variant must be 0, 1 or 2"); return CP_EINVAL; }
+    if (cfg->kernel_variant != 1 && !c->use_tc) {
         // the default variant is the tensor-core path; refuse to run it silently on
         // something else (no fallback dispatch).  Variant 1 is the explicit SIMT path.
 #ifdef CP_WITH_TC
         delete c;
-        cp_set_error("cp_create: kernel_variant 0 needs an sm_100 device");
+        cp_set_error("cp_create: kernel_variant 0 / 2 need an sm_100 device");
         return CP_EINVAL;
 #endif
     }
@@ -139,8 +143,8 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     chk(cudaMalloc(&c->d_part_ml, sizeof(float2) * (size_t)c->max_partial_rows));
     chk(cudaMalloc(&c->d_counter, sizeof(int32_t) * 4));
 #if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
-    chk(cudaMalloc(&c->d_prof, sizeof(unsigned long long) * 16 * 1024));
-    chk(cudaMemset(c->d_prof, 0, sizeof(unsigned long long) * 16 * 1024));
+    chk(cudaMalloc(&c->d_prof, sizeof(unsigned long long) * 32 * 1024));
+    chk(cudaMemset(c->d_prof, 0, sizeof(unsigned long long) * 32 * 1024));
 #endif
     chk(cudaMemset(c->d_counter, 0, sizeof(int32_t) * 4));
     for (int i = 0; i < 2; ++i) {
@@ -160,6 +164,8 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     c->items.reserve(c->max_items);
     c->sorted.reserve(c->max_items);
     c->combines.reserve(c->max_combine);
+    c->plan.reserve(2 * q_tiles);
+    c->plan_prow.reserve(q_tiles * Hkv);
     *out = c;
     return CP_OK;
 }
@@ -248,14 +254,19 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
         bool overflow = false;
         for (int j = 0; j < n_reqs && !overflow; ++j) {
             const cp_req_desc& r = reqs[j];
-            for (int q0 = 0; q0 < r.q_len && !overflow; q0 += TQ) {
-                const int qt = std::min(TQ, r.q_len - q0);
-                const int rows = qt * G;
+            // pass 1: per (q tile, KV head) group, reserve the split workspace and the combine item
+            const int nq = (r.q_len + TQ - 1) / TQ;
+            c->plan.resize((size_t)nq * 2);                          // [qi] = {n_splits, tps}
+            c->plan_prow.resize((size_t)nq * sh.Hkv);
+            int max_splits = 0;
+            for (int qi = 0; qi < nq && !overflow; ++qi) {
+                const int q0 = qi * TQ, qt = std::min(TQ, r.q_len - q0), rows = qt * G;
                 const int lim = r.ctx_off + q0 + qt;                 // causal limit of the last row
                 const int n_tiles = (lim + kKeyTile - 1) / kKeyTile;
                 const int n_splits = (n_tiles + chunk_tiles - 1) / chunk_tiles;
-                const int tps = (n_tiles + n_splits - 1) / n_splits;
-                const int kind = (c->use_tc && rows <= 16 && sh.D == 128) ? kKindSwap : kKindTile;
+                c->plan[2 * qi] = n_splits;
+                c->plan[2 * qi + 1] = (n_tiles + n_splits - 1) / n_splits;
+                max_splits = std::max(max_splits, n_splits);
                 for (int g = 0; g < sh.Hkv; ++g) {
                     int32_t prow = -1;
                     if (n_splits > 1) {
@@ -265,15 +276,28 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
                             c->combines.size() >= c->max_combine) { overflow = true; break; }
                         c->combines.push_back(CombineItem{(int32_t)(tok + q0), qt, g, n_splits, prow, {0, 0, 0}});
                     }
-                    if (c->items.size() + n_splits > c->max_items) { overflow = true; break; }
-                    for (int s = 0; s < n_splits; ++s) {
-                        const int kb = s * tps * kKeyTile;
-                        const int ke = std::min(lim, (s + 1) * tps * kKeyTile);
-                        c->items.push_back(WorkItem{j, g, q0, qt, kb, ke,
-                                                    prow < 0 ? -1 : prow + s * rows, kind});
-                    }
+                    c->plan_prow[(size_t)qi * sh.Hkv + g] = prow;
                 }
+                if (c->items.size() + (size_t)n_splits * sh.Hkv > c->max_items) overflow = true;
             }
+            // pass 2: emit in (KV head, split, q tile) order, so that the q tiles of a chunk that read
+            // the same K/V range sit next to each other in the work list, start together on
+            // neighbouring SMs and share those K/V tiles in L2 (one DRAM fetch for all of them)
+            size_t emitted = 0;
+            for (int g = 0; g < sh.Hkv && !overflow; ++g)
+                for (int s = 0; s < max_splits && !overflow; ++s)
+                    for (int qi = 0; qi < nq; ++qi) {
+                        if (s >= c->plan[2 * qi]) continue;
+                        const int q0 = qi * TQ, qt = std::min(TQ, r.q_len - q0), rows = qt * G;
+                        const int lim = r.ctx_off + q0 + qt, tps = c->plan[2 * qi + 1];
+                        const int kind = (c->use_tc && rows <= 16 && sh.D == 128) ? kKindSwap : kKindTile;
+                        const int32_t prow = c->plan_prow[(size_t)qi * sh.Hkv + g];
+                        if (c->items.size() >= c->max_items) { overflow = true; break; }
+                        c->items.push_back(WorkItem{j, g, q0, qt, s * tps * kKeyTile, std::min(lim, (s + 1) * tps * kKeyTile),
+                                                    prow < 0 ? -1 : prow + s * rows, kind});
+                        ++emitted;
+                    }
+            (void)emitted;
             tok += r.q_len;
         }
         if (!overflow) break;
@@ -281,15 +305,22 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
         chunk_tiles *= 2;                                            // coarser splits need less workspace
     }
 
-    // ---- LPT order: bucket sort by descending number of key tiles -------------------------
+    // ---- LPT order: bucket sort by descending number of key tiles.  The dual-lane kernel takes the
+    // tile-kind items first and the swap-kind items after them (two lists, one array).
     const size_t n_items = c->items.size();
     int max_cost = 0;
-    for (const WorkItem& w : c->items) max_cost = std::max(max_cost, (w.kv_end - w.kv_begin + kKeyTile - 1) / kKeyTile);
-    c->bucket.assign((size_t)max_cost + 2, 0);
-    for (const WorkItem& w : c->items) ++c->bucket[(size_t)(max_cost - (w.kv_end - w.kv_begin + kKeyTile - 1) / kKeyTile) + 1];
+    int32_t n_tile_items = 0;
+    // cost = key tiles, in steps of 4: LPT needs no finer order, and items of nearly equal length keep
+    // their emission order (the L2-sharing neighbourhoods above)
+    auto cost_of = [](const WorkItem& w) { return (w.kv_end - w.kv_begin + 4 * kKeyTile - 1) / (4 * kKeyTile); };
+    for (const WorkItem& w : c->items) { max_cost = std::max(max_cost, cost_of(w)); n_tile_items += w.kind == kKindTile; }
+    const size_t kind_stride = c->use_dl ? (size_t)max_cost + 1 : 0;
+    auto bucket_of = [&](const WorkItem& w) { return (w.kind == kKindSwap ? kind_stride : 0) + (size_t)(max_cost - cost_of(w)); };
+    c->bucket.assign(kind_stride + (size_t)max_cost + 2, 0);
+    for (const WorkItem& w : c->items) ++c->bucket[bucket_of(w) + 1];
     for (size_t i = 1; i < c->bucket.size(); ++i) c->bucket[i] += c->bucket[i - 1];
     c->sorted.resize(n_items);
-    for (const WorkItem& w : c->items) c->sorted[c->bucket[(size_t)(max_cost - (w.kv_end - w.kv_begin + kKeyTile - 1) / kKeyTile)]++] = w;
+    for (const WorkItem& w : c->items) c->sorted[c->bucket[bucket_of(w)]++] = w;
 
     // ---- pack into pinned staging ------------------------------------------------------------
     const int si = c->stage_idx ^ 1;
@@ -345,6 +376,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     m.n_tokens = (int32_t)T;
     m.n_work = (int32_t)n_items;
     m.n_combine = (int32_t)c->combines.size();
+    m.n_tile = n_tile_items;
 
     int32_t n_tc = 0;
     if (c->use_tc) n_tc = (int32_t)n_items;
@@ -427,13 +459,18 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
     if (rc != CP_OK) return rc;
     if (!c->tc_attr_set) {
         CP_CUDA(cudaFuncSetAttribute(attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcLayout<D>::kTotal));
+        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D>::kTotal));
         c->tc_attr_set = true;
     }
     if (m.n_work > 0) {
-        TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
-        int grid = std::min(c->n_sm, m.n_work);
-        if (const char* e = getenv("CP_TC_GRID")) grid = std::max(1, std::min(grid, atoi(e)));   // experiments only
-        attn_tc_kernel<D><<<grid, kTcThreads, TcLayout<D>::kTotal, stream>>>(p, *tmap);
+        const int grid = std::min(c->n_sm, m.n_work);
+        if (c->use_dl) {
+            dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
+            dl::attn_dl_kernel<D><<<grid, dl::kThreads, dl::Layout<D>::kTotal, stream>>>(p, *tmap);
+        } else {
+            TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
+            attn_tc_kernel<D><<<grid, kTcThreads, TcLayout<D>::kTotal, stream>>>(p, *tmap);
+        }
         CP_CUDA(cudaGetLastError());
         ++*launches;
         c->info.grid_attn = grid;
@@ -546,7 +583,7 @@ extern "C" int cp_set_memory_stats(cp_ctx* c, float used, float freemb, float al
 extern "C" int cp_debug_prof(cp_ctx* c, unsigned long long* host_buf, int n_ctas) {
     if (!c->d_prof) return CP_ESTATE;
     cudaDeviceSynchronize();
-    return cudaMemcpy(host_buf, c->d_prof, sizeof(unsigned long long) * 16 * n_ctas, cudaMemcpyDeviceToHost) == cudaSuccess ? CP_OK : CP_ECUDA;
+    return cudaMemcpy(host_buf, c->d_prof, sizeof(unsigned long long) * 32 * n_ctas, cudaMemcpyDeviceToHost) == cudaSuccess ? CP_OK : CP_ECUDA;
 }
 #endif
 

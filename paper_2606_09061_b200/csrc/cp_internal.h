@@ -52,6 +52,7 @@ struct BatchMeta {
     const CombineItem* combine;  // [n_combine]
     const int32_t* tok_req;      // [T] request of each token (for the append kernel)
     int32_t n_reqs, n_tokens, n_work, n_combine;
+    int32_t n_tile;              // dual-lane kernel: work[0, n_tile) are tile-kind items, the rest swap-kind
 };
 
 struct Shape {

@@ -12,8 +12,11 @@
 // shared memory, its TMEM columns and its mbarriers; the lanes share nothing but the SM.
 //
 //   warpgroup 0: warp 0 producer T, warp 1 producer S, warp 2 MMA T, warp 3 MMA S  (64 regs)
-//   warpgroup 1: softmax T (thread <-> Q-tile row)                                 (224 regs)
-//   warpgroup 2: softmax S (thread <-> key of the tile)                            (128 regs)
+//   warpgroup 1: softmax T (thread <-> Q-tile row; also the decode items lane T runs once the
+//                tile list is exhausted: thread <-> key)                            (232 regs)
+//   warpgroup 2: softmax S (thread <-> key of the tile)                            (160 regs)
+// (Measured alternatives, round 1: splitting a score tile over two softmax warpgroups, and
+// reading the score row in chunks, were no faster -- see DESIGN.md section 6.)
 //
 //   kKindTile   S[128 rows x 128 keys] = Q K^T with Q held in TMEM (A operand from TMEM, written
 //               once per item with tcgen05.st), P written back over S in TMEM as bf16 and consumed
@@ -39,8 +42,8 @@ constexpr int kItemRing = 2;
 constexpr int kTmemCols = 512;
 // TMEM columns.  Lane T: S0, S1 (fp32 scores, P aliased over their first 64 columns), O, Q.
 // Lane S: 16-column S^T0, S^T1, O^T.
-constexpr uint32_t kColS[2][2] = {{0, 128}, {448, 464}};
-constexpr uint32_t kColO[2] = {256, 480};
+__host__ __device__ constexpr uint32_t col_s(int lane, uint32_t buf) { return lane == 0 ? buf * 128u : 448u + buf * 16u; }
+__host__ __device__ constexpr uint32_t col_o(int lane) { return lane == 0 ? 256u : 480u; }
 constexpr uint32_t kColQ = 384;
 constexpr float kRescaleThreshold = 8.0f;      // log2 units: rescale O only when the max grew > 2^8
 constexpr uint32_t kSmallBytes = 12288;        // per lane: Q^T (4 KiB) + double-buffered P^T (8 KiB)
@@ -60,18 +63,32 @@ struct Layout {
     static constexpr uint32_t kTotal = kOffMisc + kMiscBytes + 1024;   // + slack to align the base to 1024
 };
 
+// Optional role-level wait-time profile of lane T (build with -DCP_TC_PROF; debugging aid only).
+#ifdef CP_TC_PROF
+#define DL_T0 long long t0__ = clock64()
+#define DL_ACC(id) do { const long long t1__ = clock64(); if ((threadIdx.x & 31) == 0) atomicAdd(&ls->prof[id], (unsigned long long)(t1__ - t0__)); t0__ = t1__; } while (0)
+#else
+#define DL_T0 do {} while (0)
+#define DL_ACC(id) do {} while (0)
+#endif
+
 struct LaneState {              // one per lane, in the misc region
     uint64_t kv_full[kMaxStages];
     uint64_t kv_empty[kMaxStages];
-    uint64_t q_full;
+    // q_full / p_full exist per item kind ("set" 0 = tile kind, set 1 = swap kind), each with its
+    // own phase counters; lane S uses set 1 only
+    uint64_t q_full[2];
     uint64_t s_full[2];
-    uint64_t p_full[2];         // indexed by tile parity: a waiter can never be two phases behind
+    uint64_t p_full[2][2];      // [set][tile parity]: a waiter can never be two phases behind
     uint64_t pv_done[2];        // PV of tile gt completes on pv_done[gt & 1]
     uint64_t item_full[kItemRing];
     uint64_t item_empty[kItemRing];
     WorkItem items[kItemRing];  // published by the lane's producer; kind < 0 = no more work
     float cmax[2][4][16];       // swap kind: per-warp column maxima, double buffered
     float lsum[4][16];          // swap kind: per-warp column sums at the end of an item
+#ifdef CP_TC_PROF
+    unsigned long long prof[16];
+#endif
 };
 
 struct Misc {
@@ -88,6 +105,7 @@ struct Params {
     float* part_o;
     float2* part_ml;
     int32_t* counters;          // [0] next tile item, [1] next swap item, [2] finished CTAs
+    unsigned long long* prof;   // [grid][16] role wait-time profile (-DCP_TC_PROF builds), else unused
 };
 
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
@@ -129,9 +147,18 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
         if (tiles_left) {
             if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
             idx = __shfl_sync(0xffffffffu, idx, 0);
-            if (idx >= p.meta.n_tile) { tiles_left = false; idx = -1; }
+            if (idx >= p.meta.n_tile) {
+                tiles_left = false; idx = -1;
+#ifdef CP_TC_PROF
+                if (lane == 0) ls->prof[13] = (unsigned long long)clock64();      // lane T: tile list exhausted (absolute clock)
+#endif
+            }
         }
+#ifdef DL_X_NO_LANE_S
+        if (idx < 0 && LANE == 0) {
+#else
         if (idx < 0) {
+#endif
             if (lane == 0) idx = atomicAdd(&p.counters[1], 1);
             idx = __shfl_sync(0xffffffffu, idx, 0);
             idx = idx < p.meta.n_work - p.meta.n_tile ? idx + p.meta.n_tile : -1;
@@ -173,7 +200,7 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             const int n_pages = min(8, n_pages_item - tile * 8);          // 1..8
             const uint32_t ld = ld_base + i;
             const uint32_t slot = ld % kStages;
-            ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1);
+            { DL_T0; ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1); DL_ACC(8); }
             const bool leader = ptx::elect_one();
             if (leader) ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u);
             uint8_t* dst = kv_base + slot * L::kSlotBytes;
@@ -188,6 +215,9 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             __syncwarp();
         }
         ld_base += 2 * n_tiles;
+#ifdef CP_TC_PROF
+        if (lane == 0 && __shfl_sync(1u, w, 7) == kKindSwap) ls->prof[14] += (unsigned long long)n_tiles;   // swap tiles streamed by this lane
+#endif
     }
 }
 
@@ -197,7 +227,7 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
 // ------------------------------------------------------------------------------------------
 template <int D, int LANE>
 __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
-                                         uint32_t& cons_cnt, uint32_t& gt, uint32_t item_cnt) {
+                                         uint32_t& cons_cnt, uint32_t& gt, uint32_t (&gp)[2], uint32_t (&ic)[2]) {
     using L = Layout<D>;
     constexpr int kStages = LANE == 0 ? kStagesT : kStagesS;
     const int n_tiles = (__shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0) + kKeyTile - 1) / kKeyTile;
@@ -209,15 +239,19 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
     const uint32_t idesc_pv = swap ? ptx::umma_idesc_bf16(128, 16, true, false) : ptx::umma_idesc_bf16(128, D, false, true);
     const uint32_t small_half = 2048;          // 16 rows x 128 B (Q^T / P^T halves in the swap kind)
 
-    ptx::mbar_wait(&ls->q_full, item_cnt & 1);
+    const int set = swap ? 1 : 0;              // barrier set and phase counters of this item kind
+    { DL_T0; ptx::mbar_wait(&ls->q_full[set], ic[set] & 1); DL_ACC(7); }
     ptx::tc_fence_after();
+    ++ic[set];
 
     auto issue_qk = [&](uint32_t g) {          // g: global tile counter of the tile being scored
         const uint32_t slot = cons_cnt % kStages, buf = g & 1;
+        DL_T0;
         ptx::mbar_wait(&ls->kv_full[slot], (cons_cnt / kStages) & 1);
+        DL_ACC(4);
         ptx::tc_fence_after();
         const uint32_t k_tile = kv_base + slot * L::kSlotBytes;
-        const uint32_t d_tmem = tmem + kColS[LANE][buf];
+        const uint32_t d_tmem = tmem + col_s(LANE, buf);
         if (ptx::elect_one()) {
 #pragma unroll
             for (int ks = 0; ks < D / 16; ++ks) {
@@ -234,23 +268,28 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
             ptx::umma_commit(&ls->s_full[buf]);
         }
         __syncwarp();
+        DL_ACC(11);
         ++cons_cnt;
     };
     auto issue_pv = [&](bool first) {
         const uint32_t buf = gt & 1;
-        ptx::mbar_wait(&ls->p_full[buf], (gt >> 1) & 1);
+        DL_T0;
+        ptx::mbar_wait(&ls->p_full[set][gp[set] & 1], (gp[set] >> 1) & 1);
+        DL_ACC(5);
+        ++gp[set];
         const uint32_t slot = cons_cnt % kStages;
         ptx::mbar_wait(&ls->kv_full[slot], (cons_cnt / kStages) & 1);
+        DL_ACC(6);
         ptx::tc_fence_after();
         const uint32_t v_tile = kv_base + slot * L::kSlotBytes;
-        const uint32_t d_tmem = tmem + kColO[LANE];
+        const uint32_t d_tmem = tmem + col_o(LANE);
         if (ptx::elect_one()) {
 #pragma unroll
             for (int ks = 0; ks < kKeyTile / 16; ++ks) {
                 // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
                 const uint64_t v_desc = ptx::umma_desc_sw128(v_tile + ks * L::kPageBytes, 1024, L::kGroupBytes);
                 if (LANE == 0 && !swap) {
-                    umma_ts(d_tmem, tmem + kColS[0][buf] + ks * 8, v_desc, idesc_pv, !first || ks > 0);
+                    umma_ts(d_tmem, tmem + col_s(0, buf) + ks * 8, v_desc, idesc_pv, !first || ks > 0);
                 } else {
                     const uint32_t poff = 4096 + buf * 4096 + (ks >> 2) * small_half + (ks & 3) * 32;   // P^T is double buffered
                     ptx::umma_ss(d_tmem, v_desc, ptx::umma_desc_sw128(small + poff, 16, 1024), idesc_pv, !first || ks > 0);
@@ -260,13 +299,14 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
             ptx::umma_commit(&ls->pv_done[buf]);
         }
         __syncwarp();
+        DL_ACC(12);
         ++cons_cnt;
         ++gt;
     };
 
     // QK(k+1) is issued before PV(k) so the softmax of tile k overlaps the next score MMA.  p_full is
-    // indexed by tile parity: the softmax of tile k+2 needs QK(k+2), which is issued only after
-    // p_full[k & 1] of tile k was observed here, so a wait can never alias onto a later phase.
+    // indexed by tile parity (per item kind): the softmax of tile k+2 needs QK(k+2), which is issued
+    // only after p_full of tile k was observed here, so a wait can never alias onto a later phase.
     issue_qk(gt);
     for (int k = 0; k < n_tiles; ++k) {
         if (k + 1 < n_tiles) issue_qk(gt + 1);
@@ -278,7 +318,7 @@ template <int D, int LANE>
 __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lane) {
     LaneState* ls = &misc->lane[LANE];
     const uint32_t tmem = misc->tmem_base;
-    uint32_t cons_cnt = 0, gt = 0, item_cnt = 0;
+    uint32_t cons_cnt = 0, gt = 0, item_cnt = 0, gp[2] = {0, 0}, ic[2] = {0, 0};
     for (;;) {
         const uint32_t islot = item_cnt % kItemRing;
         ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1);
@@ -286,7 +326,411 @@ __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lan
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&ls->item_empty[islot]);
         if (it.kind < 0) break;
-        mma_item<D, LANE>(it, smem_base, ls, tmem, cons_cnt, gt, item_cnt);
+        mma_item<D, LANE>(it, smem_base, ls, tmem, cons_cnt, gt, gp, ic);
         ++item_cnt;
     }
 }
+
+// ------------------------------------------------------------------------------------------
+// softmax warpgroup of lane T, tile kind: thread <-> row of the 128-row Q tile.  Q row -> TMEM once,
+// then per key tile: the whole score row from TMEM in ONE load batch (a tcgen05.ld/wait round trip
+// costs ~70 cycles per warp that has one in flight, whatever its size, so it is issued once per
+// tile), online softmax (log2 domain, lazy rescale), P row -> TMEM over the first 64 columns of the
+// same S buffer (bf16 pairs), O rescale / epilogue from TMEM.
+// ------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p, LaneState* ls, uint32_t tmem,
+                                             uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base) {
+    const Shape& sh = p.sh;
+    const int G = sh.G;
+    const int R = it.q_tokens * G;
+    const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
+    const int tok0 = p.meta.cu_q[it.req] + it.q_start;
+    const int ctx = p.meta.ctx_off[it.req];
+    const bool valid_row = row < R;
+    const int tok = tok0 + row / G;
+    const int head = it.kv_head * G + row % G;
+    const float scale = sh.sm_scale * 1.4426950408889634f;
+    const uint32_t t_row = tmem + (lane_base << 16);
+
+    DL_T0;
+    // ---- Q row -> TMEM (A operand of QK^T): column j holds elements (2j, 2j+1)
+    {
+        const uint4* src = reinterpret_cast<const uint4*>(p.q + ((int64_t)tok * sh.Hq + head) * D);
+#pragma unroll
+        for (int c = 0; c < D / 64; ++c) {
+            uint32_t r[32];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const uint4 v = valid_row ? src[c * 8 + j] : make_uint4(0, 0, 0, 0);
+                r[4 * j] = v.x; r[4 * j + 1] = v.y; r[4 * j + 2] = v.z; r[4 * j + 3] = v.w;
+            }
+            ptx::tmem_st32(t_row + kColQ + c * 32, r);
+        }
+        ptx::tmem_wait_st();
+        ptx::tc_fence_before();
+        ptx::mbar_arrive(&ls->q_full[0]);
+    }
+    DL_ACC(9);
+
+    const int limit = valid_row ? min(it.kv_end, ctx + it.q_start + row / G + 1) : 0;   // causal, diagonal inclusive
+    float m_ref = -INFINITY, l = 0.f;
+
+    for (int k = 0; k < n_tiles; ++k) {
+        const int ts = it.kv_begin + k * kKeyTile;
+        const uint32_t buf = gt & 1;
+        const uint32_t t_s = t_row + col_s(0, buf);
+        ptx::mbar_wait(&ls->s_full[buf], (gt >> 1) & 1);
+        DL_ACC(0);
+        ptx::tc_fence_after();
+        uint32_t sr[128];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) ptx::tmem_ld32(t_s + c * 32, sr + c * 32);
+        ptx::tmem_wait_ld();
+        const int nvalid = max(0, min(kKeyTile, limit - ts));
+        float mx[8];                                    // 8 independent max chains
+#pragma unroll
+        for (int i = 0; i < 8; ++i) mx[i] = -INFINITY;
+        if (nvalid == kKeyTile) {
+#pragma unroll
+            for (int j = 0; j < 128; ++j) mx[j & 7] = fmaxf(mx[j & 7], __uint_as_float(sr[j]));
+        } else {
+#pragma unroll
+            for (int j = 0; j < 128; ++j) mx[j & 7] = fmaxf(mx[j & 7], j < nvalid ? __uint_as_float(sr[j]) : -INFINITY);
+        }
+        float m_t = fmaxf(fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])), fmaxf(fmaxf(mx[4], mx[5]), fmaxf(mx[6], mx[7])));
+        m_t *= scale;                                   // scale > 0
+        float alpha = 1.f;
+        bool rescale = false;
+        if (m_t > m_ref + kRescaleThreshold) {          // also the first finite max (m_ref = -inf)
+            alpha = (m_ref == -INFINITY) ? 0.f : ptx::ex2(m_ref - m_t);
+            m_ref = m_t;
+            rescale = true;
+        }
+        const float neg_m = (m_ref == -INFINITY) ? 0.f : -m_ref;
+        float sm[4] = {0.f, 0.f, 0.f, 0.f};             // independent sum chains
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {                   // 32 scores -> 16 packed P columns
+            uint32_t pk[16];
+            if (nvalid == kKeyTile) {
+#pragma unroll
+                for (int j = 0; j < 32; j += 2) {
+                    const float a = ptx::ex2(fmaf(__uint_as_float(sr[c * 32 + j]), scale, neg_m));
+                    const float b = ptx::ex2(fmaf(__uint_as_float(sr[c * 32 + j + 1]), scale, neg_m));
+                    sm[(j >> 1) & 3] += a + b;
+                    pk[j >> 1] = pack_bf16(a, b);
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < 32; j += 2) {
+                    const int key = c * 32 + j;
+                    const float a = key < nvalid ? ptx::ex2(fmaf(__uint_as_float(sr[key]), scale, neg_m)) : 0.f;
+                    const float b = key + 1 < nvalid ? ptx::ex2(fmaf(__uint_as_float(sr[key + 1]), scale, neg_m)) : 0.f;
+                    sm[(j >> 1) & 3] += a + b;
+                    pk[j >> 1] = pack_bf16(a, b);
+                }
+            }
+            ptx::tmem_st16(t_s + c * 16, pk);
+        }
+        l = l * alpha + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
+        if (k > 0 && __any_sync(0xffffffffu, rescale)) {
+            ptx::mbar_wait(&ls->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);      // PV(k-1) done: O readable
+            ptx::tc_fence_after();
+#pragma unroll 1
+            for (int c = 0; c < D / 32; ++c) {
+                uint32_t o[32];
+                ptx::tmem_ld32(t_row + col_o(0) + c * 32, o);
+                ptx::tmem_wait_ld();
+#pragma unroll
+                for (int j = 0; j < 32; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+                ptx::tmem_st32(t_row + col_o(0) + c * 32, o);
+            }
+        }
+        ptx::tmem_wait_st();
+        ptx::tc_fence_before();
+        ptx::mbar_arrive(&ls->p_full[0][gp & 1]);
+        DL_ACC(1);
+        ++gt;
+        ++gp;
+    }
+
+    // ---- epilogue: O row from TMEM (one load batch) -> out (bf16, normalised) or split workspace (fp32, unnormalised)
+    ptx::mbar_wait(&ls->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
+    DL_ACC(2);
+    ptx::tc_fence_after();
+    const float inv = 1.f / l;
+    uint32_t o[D];
+#pragma unroll
+    for (int c = 0; c < D / 32; ++c) ptx::tmem_ld32(t_row + col_o(0) + c * 32, o + c * 32);
+    ptx::tmem_wait_ld();
+    if (valid_row) {
+        if (it.partial_row < 0) {
+            uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * sh.Hq + head) * D);
+#pragma unroll
+            for (int j = 0; j < D / 8; ++j)
+                dst[j] = make_uint4(pack_bf16(__uint_as_float(o[8 * j]) * inv, __uint_as_float(o[8 * j + 1]) * inv),
+                                    pack_bf16(__uint_as_float(o[8 * j + 2]) * inv, __uint_as_float(o[8 * j + 3]) * inv),
+                                    pack_bf16(__uint_as_float(o[8 * j + 4]) * inv, __uint_as_float(o[8 * j + 5]) * inv),
+                                    pack_bf16(__uint_as_float(o[8 * j + 6]) * inv, __uint_as_float(o[8 * j + 7]) * inv));
+        } else {
+            uint4* dst = reinterpret_cast<uint4*>(p.part_o + ((int64_t)it.partial_row + row) * D);
+#pragma unroll
+            for (int j = 0; j < D / 4; ++j) dst[j] = make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+            p.part_ml[(int64_t)it.partial_row + row] = make_float2(m_ref, l);
+        }
+    }
+    ptx::tc_fence_before();
+    DL_ACC(3);
+}
+
+// ------------------------------------------------------------------------------------------
+// softmax warps, swap kind (D = 128, R <= RC <= 16 rows): thread <-> key of the tile (S^T lane)
+// during the key loop, thread <-> d (O^T lane) for rescale / epilogue.  Column c = (token, head)
+// row; columns in [R, RC) are computed as fully masked.  Straight-line code per column so the
+// independent chains interleave; the column max is one REDUX per column and warp.
+// ------------------------------------------------------------------------------------------
+template <int LANE, int RC>
+__device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p, uint8_t* small, LaneState* ls,
+                                             uint32_t tmem, uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base, int swarp) {
+    constexpr int D = 128;
+    const Shape& sh = p.sh;
+    const int G = sh.G;
+    const int R = it.q_tokens * G;                       // <= RC
+    const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
+    const int tok0 = p.meta.cu_q[it.req] + it.q_start;
+    const int ctx = p.meta.ctx_off[it.req];
+    const float scale = sh.sm_scale * 1.4426950408889634f;
+    const int lane = row & 31;
+
+    // ---- Q^T -> smem: B operand [16 rows][D], K-major, 128B swizzle, halves 2 KB apart
+    for (int id = row; id < RC * (D / 8); id += 128) {
+        const int r = id >> 4, c = id & 15;
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (r < R) {
+            const int tok = tok0 + r / G, head = it.kv_head * G + r % G;
+            v = *reinterpret_cast<const uint4*>(p.q + ((int64_t)tok * sh.Hq + head) * D + c * 8);
+        }
+        *reinterpret_cast<uint4*>(small + (c >> 3) * 2048 + r * 128 + (((c & 7) ^ (r & 7)) << 4)) = v;
+    }
+    ptx::fence_proxy_async_smem();
+    ptx::mbar_arrive(&ls->q_full[1]);
+
+    float m_ref[RC], l_part[RC];
+    int limit[RC];
+#pragma unroll
+    for (int c = 0; c < RC; ++c) {
+        m_ref[c] = -INFINITY;
+        l_part[c] = 0.f;
+        limit[c] = c < R ? min(it.kv_end, ctx + it.q_start + c / G + 1) : 0;
+    }
+    const uint32_t t_row = tmem + (lane_base << 16);
+    // P^T element (col c, key `row`): B operand [16 rows][128 keys], K-major, halves (64 keys) 2 KB apart
+    uint8_t* pt = small + 4096 + (row >> 6) * 2048 + (row & 7) * 2;
+    const int pchunk = (row & 63) >> 3;
+
+    for (int k = 0; k < n_tiles; ++k) {
+        const int key = it.kv_begin + k * kKeyTile + row;
+        const uint32_t buf = gt & 1;
+        ptx::mbar_wait(&ls->s_full[buf], (gt >> 1) & 1);
+        ptx::tc_fence_after();
+        uint32_t sr[RC];
+        ptx::tmem_ld<RC>(t_row + col_s(LANE, buf), sr);
+        ptx::tmem_wait_ld();
+        float sv[RC];
+        int* cm = reinterpret_cast<int*>(&ls->cmax[k & 1][swarp][0]);
+#pragma unroll
+        for (int c = 0; c < RC; ++c) {
+            sv[c] = key < limit[c] ? __uint_as_float(sr[c]) * scale : -INFINITY;
+            const int w = __reduce_max_sync(0xffffffffu, ptx::f2ord(sv[c]));
+            if (lane == 0) cm[c] = w;
+        }
+        ptx::named_bar_sync(1 + LANE, 128);
+        bool any_rescale = false;
+        float alpha[RC];
+        const int* cm0 = reinterpret_cast<const int*>(&ls->cmax[k & 1][0][0]);
+#pragma unroll
+        for (int c = 0; c < RC; ++c) {
+            const float m_t = ptx::ord2f(max(max(cm0[c], cm0[16 + c]), max(cm0[32 + c], cm0[48 + c])));
+            alpha[c] = 1.f;
+            if (m_t > m_ref[c] + kRescaleThreshold) {
+                alpha[c] = (m_ref[c] == -INFINITY) ? 0.f : ptx::ex2(m_ref[c] - m_t);
+                m_ref[c] = m_t;
+                any_rescale = true;
+            }
+            const float pc = key < limit[c] ? ptx::ex2(sv[c] - m_ref[c]) : 0.f;
+            l_part[c] = l_part[c] * alpha[c] + pc;
+            sv[c] = pc;
+        }
+        if (k >= 2) {                                    // PV(gt-2) done: this P^T buffer is free again
+            ptx::mbar_wait(&ls->pv_done[buf], ((gt - 2) >> 1) & 1);
+        }
+        {
+            uint8_t* ptb = pt + buf * 4096;
+#pragma unroll
+            for (int c = 0; c < RC; ++c)
+                *reinterpret_cast<__nv_bfloat16*>(ptb + c * 128 + ((pchunk ^ (c & 7)) << 4)) = __float2bfloat16_rn(sv[c]);
+        }
+        if (k > 0 && any_rescale) {                      // uniform over the 128 threads
+            ptx::mbar_wait(&ls->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
+            ptx::tc_fence_after();
+            uint32_t o[RC];
+            ptx::tmem_ld<RC>(t_row + col_o(LANE), o);
+            ptx::tmem_wait_ld();
+#pragma unroll
+            for (int c = 0; c < RC; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha[c]);
+            ptx::tmem_st<RC>(t_row + col_o(LANE), o);
+            ptx::tmem_wait_st();
+        }
+#ifndef DL_X_S_NOFENCE
+        ptx::fence_proxy_async_smem();
+#endif
+        ptx::tc_fence_before();
+        ptx::mbar_arrive(&ls->p_full[1][gp & 1]);
+        ++gt;
+        ++gp;
+    }
+
+    // ---- column sums over the 128 key lanes
+#pragma unroll
+    for (int c = 0; c < RC; ++c) {
+        float w = l_part[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
+        if (lane == 0) ls->lsum[swarp][c] = w;
+    }
+    ptx::named_bar_sync(1 + LANE, 128);
+    // ---- epilogue: O^T[d = row][c] -> out / workspace
+    ptx::mbar_wait(&ls->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
+    ptx::tc_fence_after();
+    uint32_t o[RC];
+    ptx::tmem_ld<RC>(t_row + col_o(LANE), o);
+    ptx::tmem_wait_ld();
+#pragma unroll
+    for (int c = 0; c < RC; ++c) {
+        if (c < R) {
+            const float lc = ls->lsum[0][c] + ls->lsum[1][c] + ls->lsum[2][c] + ls->lsum[3][c];
+            if (it.partial_row < 0) {
+                const int tok = tok0 + c / G, head = it.kv_head * G + c % G;
+                p.out[((int64_t)tok * sh.Hq + head) * D + row] = __float2bfloat16_rn(__uint_as_float(o[c]) / lc);
+            } else {
+                p.part_o[((int64_t)it.partial_row + c) * D + row] = __uint_as_float(o[c]);
+                if (row == c) p.part_ml[(int64_t)it.partial_row + c] = make_float2(m_ref[c], lc);
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    ptx::named_bar_sync(1 + LANE, 128);                  // lsum / cmax are reused by the next item
+}
+
+// softmax warpgroup loop.  ROLE 0: lane T (tile kind, and the swap-kind items lane T picks up);
+// ROLE 2: lane S.
+template <int D, int ROLE>
+__device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Misc* misc, int warp, int lane) {
+    using L = Layout<D>;
+    constexpr int LANE = ROLE == 2 ? 1 : 0;
+    LaneState* ls = &misc->lane[LANE];
+    const uint32_t tmem = misc->tmem_base;
+    const uint32_t lane_base = (warp & 3) * 32;
+    const int row = lane_base + lane;
+    uint8_t* small = smem + L::kOffSmall[LANE];
+    uint32_t gt = 0, item_cnt = 0, gp_tile = 0, gp_swap = 0;
+    for (;;) {
+        const uint32_t islot = item_cnt % kItemRing;
+        { DL_T0; ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1); DL_ACC(10); }
+        const WorkItem it = ls->items[islot];
+        ptx::mbar_arrive(&ls->item_empty[islot]);
+        if (it.kind < 0) break;
+        if (ROLE == 2 || it.kind == kKindSwap) {
+            if constexpr (D == 128) {
+                const int R = it.q_tokens * p.sh.G;
+                if (R <= 4) softmax_swap<LANE, 4>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
+                else if (R <= 8) softmax_swap<LANE, 8>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
+                else softmax_swap<LANE, 16>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
+            }
+        } else {
+            if constexpr (ROLE == 0) softmax_tile<D>(it, p, ls, tmem, gt, gp_tile, row, lane_base);
+        }
+        ++item_cnt;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// the kernel
+// ------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1)
+attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
+    using L = Layout<D>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    Misc* misc = reinterpret_cast<Misc*>(smem + L::kOffMisc);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int ln = 0; ln < 2; ++ln) {
+            LaneState* ls = &misc->lane[ln];
+            for (int i = 0; i < kMaxStages; ++i) { ptx::mbar_init(&ls->kv_full[i], 1); ptx::mbar_init(&ls->kv_empty[i], 1); }
+            ptx::mbar_init(&ls->q_full[0], 128);
+            ptx::mbar_init(&ls->q_full[1], 128);
+            for (int i = 0; i < 2; ++i) {
+                ptx::mbar_init(&ls->s_full[i], 1);
+                ptx::mbar_init(&ls->p_full[0][i], 128);
+                ptx::mbar_init(&ls->p_full[1][i], 128);
+                ptx::mbar_init(&ls->pv_done[i], 1);
+            }
+            // consumers of the item ring: the lane's 128 softmax threads + its MMA warp
+            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], 128 + 1); }
+        }
+        ptx::fence_barrier_init();
+        ptx::prefetch_tmap(&tmap);
+    }
+    if (warp == 2) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
+#ifdef CP_TC_PROF
+    if (threadIdx.x < 32) misc->lane[threadIdx.x >> 4].prof[threadIdx.x & 15] = 0;
+    const long long t_start__ = clock64();
+#endif
+    // stale shared memory may hold NaN bit patterns; tiles are only partly overwritten by short
+    // requests, and 0 x NaN would poison the accumulators
+    for (uint32_t i = threadIdx.x * 16; i < L::kOffMisc; i += kThreads * 16)
+        *reinterpret_cast<uint4*>(smem + i) = make_uint4(0, 0, 0, 0);
+    ptx::fence_proxy_async_smem();
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+
+    // launch allocation: 168 registers per thread.  The producer / MMA warpgroup and the decode
+    // softmax give part of their share to the tile softmax (a 128-column score row in registers).
+    if (warp < 4) {
+        reg_dec<64>();
+        if (warp == 0) producer<D, 0>(p, &tmap, smem, &misc->lane[0], lane);
+        else if (warp == 1) producer<D, 1>(p, &tmap, smem, &misc->lane[1], lane);
+        else if (warp == 2) mma_warp<D, 0>(ptx::smem_u32(smem), misc, lane);
+        else mma_warp<D, 1>(ptx::smem_u32(smem), misc, lane);
+    } else if (warp < 8) {
+        reg_inc<232>();
+        softmax_warps<D, 0>(p, smem, misc, warp, lane);
+    } else {
+        reg_dec<160>();
+        softmax_warps<D, 2>(p, smem, misc, warp, lane);
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 2) ptx::tmem_dealloc(misc->tmem_base, kTmemCols);
+#ifdef CP_TC_PROF
+    if (threadIdx.x == 0) { misc->lane[0].prof[15] = (unsigned long long)(clock64() - t_start__); misc->lane[0].prof[13] -= (unsigned long long)t_start__; }
+    __syncthreads();
+    if (threadIdx.x < 32 && p.prof) p.prof[blockIdx.x * 32 + threadIdx.x] = misc->lane[threadIdx.x >> 4].prof[threadIdx.x & 15];
+#endif
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&p.counters[2], 1) == (int)gridDim.x - 1) {      // last CTA re-arms the counters
+            p.counters[0] = 0;
+            p.counters[1] = 0;
+            p.counters[2] = 0;
+            __threadfence();
+        }
+    }
+}
+
+}  // namespace dl
+}  // namespace cp

@@ -38,7 +38,10 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
     return ok != 0;
 }
 // A wait that does not complete within ~4 s is a protocol bug: trap (the launch fails with an
-// error) instead of hanging the device.
+// error) instead of hanging the device.  The default build keeps the wait loop free of function
+// calls (an ABI call anywhere in the kernel stops ptxas from giving the warpgroups the register
+// counts they ask for with setmaxnreg); -DCP_WAIT_DIAG prints which barrier timed out.
+#ifdef CP_WAIT_DIAG
 __device__ __noinline__ void mbar_wait_slow(uint64_t* bar, uint32_t parity) {
     const long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
@@ -49,8 +52,20 @@ __device__ __noinline__ void mbar_wait_slow(uint64_t* bar, uint32_t parity) {
         }
     }
 }
+#endif
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    if (!mbar_try_wait(bar, parity)) mbar_wait_slow(bar, parity);
+    if (mbar_try_wait(bar, parity)) return;
+#ifdef CP_WAIT_DIAG
+    mbar_wait_slow(bar, parity);
+#else
+    const long long t0 = clock64();
+    while (!mbar_try_wait(bar, parity)) {
+#ifdef DL_X_NANOSLEEP
+        __nanosleep(DL_X_NANOSLEEP);
+#endif
+        if (clock64() - t0 > 8000000000LL) __trap();
+    }
+#endif
 }
 
 // ---- proxies / fences ---------------------------------------------------------------------

@@ -162,8 +162,24 @@ def config_70b(seed: int = 0) -> BatchSpec:
     return make_spec("70b", 64, 8, 128, 16, 262144, q_len, ctx_off, seed, rng)
 
 
+def _subset(spec: BatchSpec, keep, name: str) -> BatchSpec:
+    idx = [j for j in range(spec.n_reqs) if keep(spec.q_len[j])]
+    return BatchSpec(name, spec.Hq, spec.Hkv, spec.D, spec.B, spec.num_blocks, spec.q_len[idx],
+                     spec.ctx_off[idx], [spec.block_tables[j] for j in idx], spec.seed)
+
+
+def config_b2048_decodes(seed: int = 0) -> BatchSpec:
+    """The 512 decodes of configs[2] alone (profiling breakdown: the HBM-bound part)."""
+    return _subset(config_b2048(seed), lambda q: q == 1, "b2048dec")
+
+
+def config_b2048_prefill(seed: int = 0) -> BatchSpec:
+    """The 4 prefill chunks of configs[2] alone (profiling breakdown: the tensor-bound part)."""
+    return _subset(config_b2048(seed), lambda q: q > 1, "b2048pf")
+
+
 CONFIGS = {"tiny": config_tiny, "b512": config_b512, "b2048": config_b2048,
-           "70b": config_70b}
+           "70b": config_70b, "b2048dec": config_b2048_decodes, "b2048pf": config_b2048_prefill}
 
 
 def random_spec(seed: int, Hq=8, Hkv=2, D=64, B=16, n_prefill=3, n_decode=5,

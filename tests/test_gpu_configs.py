@@ -46,12 +46,12 @@ def _run_device_config(spec, variant, n_sample):
     return stats, info
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_config_b512_full(variant):
     _run_device_config(wl.config_b512(), variant, None)
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_config_b2048_sampled(variant):
     stats, info = _run_device_config(wl.config_b2048(), variant, 2048)
     assert info.n_tokens == 2048 and info.n_reqs == 516

@@ -9,7 +9,7 @@ from tests import gpu_util as gu
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = [0, 1]       # 0 = default path (tensor-core where built), 1 = SIMT reference kernels
+VARIANTS = [0, 1, 2]    # 0 = dual-lane tcgen05 kernel (default), 1 = SIMT reference kernels, 2 = single-lane tcgen05
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
