@@ -11,10 +11,11 @@
 // Each lane owns a TMA producer warp, an MMA issuer warp, four softmax warps, a K/V tile ring in
 // shared memory, its TMEM columns and its mbarriers; the lanes share nothing but the SM.
 //
-//   warpgroup 0: warp 0 producer T, warp 1 producer S, warp 2 MMA T, warp 3 MMA S  (64 regs)
-//   warpgroup 1: softmax T (thread <-> Q-tile row; also the decode items lane T runs once the
-//                tile list is exhausted: thread <-> key)                            (232 regs)
-//   warpgroup 2: softmax S (thread <-> key of the tile)                            (160 regs)
+//   warpgroups 0-1: warps 0-2 TMA producers T, warps 3-5 TMA producers S, warp 6 MMA T,
+//                   warp 7 MMA S                                                    (48 regs)
+//   warpgroup 2:    softmax T (thread <-> Q-tile row; also the decode items lane T runs once the
+//                   tile list is exhausted: thread <-> key)                         (232 regs)
+//   warpgroup 3:    softmax S (thread <-> key of the tile)                         (160 regs)
 // (Measured alternatives, round 1: splitting a score tile over two softmax warpgroups, and
 // reading the score row in chunks, were no faster -- see DESIGN.md section 6.)
 //
@@ -36,8 +37,11 @@
 namespace cp {
 namespace dl {
 
-constexpr int kThreads = 384;
+constexpr int kThreads = 512;
 constexpr int kStagesT = 3, kStagesS = 3, kMaxStages = 4;
+constexpr int kProdT = 3, kProdS = 3;         // TMA producer warps per lane (kProdT + kProdS + 2 MMA warps = 8 warps)
+// a producer waiting for slot reuse may be at most one phase behind only if kProd <= kStages
+static_assert(kProdT <= kStagesT && kProdS <= kStagesS && kProdT + kProdS == 6, "producer / stage configuration");
 constexpr int kItemRing = 2;
 constexpr int kTmemCols = 512;
 // TMEM columns.  Lane T: S0, S1 (fp32 scores, P aliased over their first 64 columns), O, Q.
@@ -128,75 +132,78 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
 }
 
 // ------------------------------------------------------------------------------------------
-// producer warp of a lane: fetches work items, publishes them to the lane's MMA and softmax
-// warps through a small smem ring, and streams the K and V tiles of each item into the lane's
-// slot ring in consumption order K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1).  It runs ahead
-// of the consumers by up to kStages tile loads, across item boundaries.  Page ids are prefetched
-// 32 at a time (one per lane, three windows) so no dependent global load sits between TMA issues.
+// producer warps of a lane.  Producer 0 fetches work items (atomic counters) and publishes them to
+// the lane's other warps through a small smem ring; all kProd producers stream the K and V tiles of
+// each item into the lane's slot ring in consumption order K0, K1, V0, K2, V1, ..., K(n-1), V(n-2),
+// V(n-1), load number ld (counted over the whole kernel) going to producer ld mod kProd.  A warp sustains one TMA box (one 4 KiB page slab)
+// per ~230 cycles, i.e. ~3700 cycles per 128-key K+V tile pair: one producer per lane caps a lane at
+// ~33 GB/s and was the bound of both lanes; the issue rate scales with the number of warps.
+// Together the producers run ahead of the consumers by up to kStages tile loads, across item
+// boundaries.  Page ids are prefetched 32 at a time (one per lane of the warp, two windows; each
+// producer's tile sequence is monotone) so no dependent global load sits between two TMA issues.
 // ------------------------------------------------------------------------------------------
 template <int D, int LANE>
-__device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tmap, uint8_t* smem, LaneState* ls, int lane) {
+__device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tmap, uint8_t* smem, LaneState* ls, int lane, int pw) {
     using L = Layout<D>;
     constexpr int kStages = LANE == 0 ? kStagesT : kStagesS;
+    constexpr int kProd = LANE == 0 ? kProdT : kProdS;
     uint8_t* kv_base = smem + L::kOffKv[LANE];
     uint32_t ld_base = 0, item_cnt = 0;          // ld_base: tile loads of all previous items
     bool tiles_left = LANE == 0;
     for (;;) {
         const uint32_t islot = item_cnt % kItemRing;
-        int idx = -1;
-        if (tiles_left) {
-            if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
-            idx = __shfl_sync(0xffffffffu, idx, 0);
-            if (idx >= p.meta.n_tile) {
-                tiles_left = false; idx = -1;
-#ifdef CP_TC_PROF
-                if (lane == 0) ls->prof[13] = (unsigned long long)clock64();      // lane T: tile list exhausted (absolute clock)
-#endif
+        int w;
+        if (pw == 0) {                           // producer 0 fetches the next item and publishes it
+            int idx = -1;
+            if (tiles_left) {
+                if (lane == 0) idx = atomicAdd(&p.counters[0], 1);
+                idx = __shfl_sync(0xffffffffu, idx, 0);
+                if (idx >= p.meta.n_tile) { tiles_left = false; idx = -1; }
             }
+            if (idx < 0) {
+                if (lane == 0) idx = atomicAdd(&p.counters[1], 1);
+                idx = __shfl_sync(0xffffffffu, idx, 0);
+                idx = idx < p.meta.n_work - p.meta.n_tile ? idx + p.meta.n_tile : -1;
+            }
+            w = 0;                               // one int32 of the 32-byte WorkItem per lane 0..7
+            if (idx >= 0 && lane < 8) w = reinterpret_cast<const int32_t*>(p.meta.work + idx)[lane];
+            if (idx < 0 && lane == 7) w = -1;    // kind = -1: sentinel
+            ptx::mbar_wait(&ls->item_empty[islot], ((item_cnt / kItemRing) & 1) ^ 1);
+            if (lane < 8) reinterpret_cast<int32_t*>(&ls->items[islot])[lane] = w;
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&ls->item_full[islot]);
+        } else {
+            ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1);
+            w = lane < 8 ? reinterpret_cast<const int32_t*>(&ls->items[islot])[lane] : 0;
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&ls->item_empty[islot]);
         }
-#ifdef DL_X_NO_LANE_S
-        if (idx < 0 && LANE == 0) {
-#else
-        if (idx < 0) {
-#endif
-            if (lane == 0) idx = atomicAdd(&p.counters[1], 1);
-            idx = __shfl_sync(0xffffffffu, idx, 0);
-            idx = idx < p.meta.n_work - p.meta.n_tile ? idx + p.meta.n_tile : -1;
-        }
-        int w = 0;                               // one int32 of the 32-byte WorkItem per lane 0..7
-        if (idx >= 0 && lane < 8) w = reinterpret_cast<const int32_t*>(p.meta.work + idx)[lane];
-        if (idx < 0 && lane == 7) w = -1;        // kind = -1: sentinel
-        ptx::mbar_wait(&ls->item_empty[islot], ((item_cnt / kItemRing) & 1) ^ 1);
-        if (lane < 8) reinterpret_cast<int32_t*>(&ls->items[islot])[lane] = w;
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&ls->item_full[islot]);
         ++item_cnt;
-        if (idx < 0) break;
+        if (__shfl_sync(0xffffffffu, w, 7) < 0) break;
         const int req = __shfl_sync(0xffffffffu, w, 0), kv_head = __shfl_sync(0xffffffffu, w, 1);
         const int kv_begin = __shfl_sync(0xffffffffu, w, 4), kv_end = __shfl_sync(0xffffffffu, w, 5);
         const int n_tiles = (kv_end - kv_begin + kKeyTile - 1) / kKeyTile;
         const int32_t* bt = p.meta.block_table + p.meta.bt_off[req] + (kv_begin >> 4);
         const int n_pages_item = (kv_end - kv_begin + 15) >> 4;
-        // page-id windows of 32 pages (4 tiles), one id per lane.  V tiles advance the window; the
-        // K stream is at most one tile ahead of the V stream, so it reads window cur_w or cur_w + 1.
+        // page-id windows of 32 pages (4 tiles), one id per lane: cur = window cur_w, nxt = the next
         int cur_w = 0;
-        int win0 = lane < n_pages_item ? bt[lane] : 0;
-        int win1 = 32 + lane < n_pages_item ? bt[32 + lane] : 0;
-        int win2 = 64 + lane < n_pages_item ? bt[64 + lane] : 0;
-        for (int i = 0; i < 2 * n_tiles; ++i) {
+        int cur = lane < n_pages_item ? bt[lane] : 0;
+        int nxt = 32 + lane < n_pages_item ? bt[32 + lane] : 0;
+        // load number ld = ld_base + i (global over the whole kernel) belongs to producer ld % kProd, so a
+        // producer's previous load is always ld - kProd: with kProd <= kStages the slot it waits for is at
+        // most one phase behind and the parity wait cannot alias
+        for (int i = (pw + kProd - (int)(ld_base % kProd)) % kProd; i < 2 * n_tiles; i += kProd) {
             int is_v, tile;
             if (i == 0) { is_v = 0; tile = 0; }
             else if (i == 2 * n_tiles - 1) { is_v = 1; tile = n_tiles - 1; }
             else if (i & 1) { is_v = 0; tile = (i + 1) >> 1; }
             else { is_v = 1; tile = (i >> 1) - 1; }
-            if (is_v && (tile >> 2) > cur_w) {
-                win0 = win1;
-                win1 = win2;
+            while ((tile >> 2) > cur_w) {
+                cur = nxt;
                 ++cur_w;
-                const int pi = (cur_w + 2) * 32 + lane;
-                win2 = pi < n_pages_item ? bt[pi] : 0;
+                const int pi = (cur_w + 1) * 32 + lane;
+                nxt = pi < n_pages_item ? bt[pi] : 0;
             }
-            const int win = (tile >> 2) == cur_w ? win0 : win1;
             const int n_pages = min(8, n_pages_item - tile * 8);          // 1..8
             const uint32_t ld = ld_base + i;
             const uint32_t slot = ld % kStages;
@@ -206,7 +213,7 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             uint8_t* dst = kv_base + slot * L::kSlotBytes;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                const int pg = __shfl_sync(0xffffffffu, win, (tile & 3) * 8 + j);
+                const int pg = __shfl_sync(0xffffffffu, cur, (tile & 3) * 8 + j);
                 if (j < n_pages) {
                     const int slab = (pg * 2 + is_v) * p.sh.Hkv + kv_head;
                     if (leader) ptx::tma_load_5d(dst + j * L::kPageBytes, tmap, &ls->kv_full[slot], 0, 0, 0, 0, slab);
@@ -215,9 +222,6 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             __syncwarp();
         }
         ld_base += 2 * n_tiles;
-#ifdef CP_TC_PROF
-        if (lane == 0 && __shfl_sync(1u, w, 7) == kKindSwap) ls->prof[14] += (unsigned long long)n_tiles;   // swap tiles streamed by this lane
-#endif
     }
 }
 
@@ -285,7 +289,11 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
         const uint32_t d_tmem = tmem + col_o(LANE);
         if (ptx::elect_one()) {
 #pragma unroll
+#ifdef DL_X_NOPV
+            for (int ks = 0; ks < 0; ++ks) {
+#else
             for (int ks = 0; ks < kKeyTile / 16; ++ks) {
+#endif
                 // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
                 const uint64_t v_desc = ptx::umma_desc_sw128(v_tile + ks * L::kPageBytes, 1024, L::kGroupBytes);
                 if (LANE == 0 && !swap) {
@@ -678,13 +686,13 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 ptx::mbar_init(&ls->p_full[1][i], 128);
                 ptx::mbar_init(&ls->pv_done[i], 1);
             }
-            // consumers of the item ring: the lane's 128 softmax threads + its MMA warp
-            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], 128 + 1); }
+            // readers of the item ring: the lane's 128 softmax threads, its MMA warp, its other producers
+            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], 128 + 1 + (ln == 0 ? kProdT : kProdS) - 1); }
         }
         ptx::fence_barrier_init();
         ptx::prefetch_tmap(&tmap);
     }
-    if (warp == 2) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
+    if (warp == 6) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
 #ifdef CP_TC_PROF
     if (threadIdx.x < 32) misc->lane[threadIdx.x >> 4].prof[threadIdx.x & 15] = 0;
     const long long t_start__ = clock64();
@@ -698,24 +706,24 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     __syncthreads();
     ptx::tc_fence_after();
 
-    // launch allocation: 168 registers per thread.  The producer / MMA warpgroup and the decode
-    // softmax give part of their share to the tile softmax (a 128-column score row in registers).
-    if (warp < 4) {
-        reg_dec<64>();
-        if (warp == 0) producer<D, 0>(p, &tmap, smem, &misc->lane[0], lane);
-        else if (warp == 1) producer<D, 1>(p, &tmap, smem, &misc->lane[1], lane);
-        else if (warp == 2) mma_warp<D, 0>(ptx::smem_u32(smem), misc, lane);
+    // launch allocation: 128 registers per thread.  The two producer / MMA warpgroups give most of
+    // their share to the tile softmax (a 128-column score row in registers) and the decode softmax.
+    if (warp < 8) {
+        reg_dec<48>();
+        if (warp < kProdT) producer<D, 0>(p, &tmap, smem, &misc->lane[0], lane, warp);
+        else if (warp < kProdT + kProdS) producer<D, 1>(p, &tmap, smem, &misc->lane[1], lane, warp - kProdT);
+        else if (warp == 6) mma_warp<D, 0>(ptx::smem_u32(smem), misc, lane);
         else mma_warp<D, 1>(ptx::smem_u32(smem), misc, lane);
-    } else if (warp < 8) {
+    } else if (warp < 12) {
         reg_inc<232>();
         softmax_warps<D, 0>(p, smem, misc, warp, lane);
     } else {
-        reg_dec<160>();
+        reg_inc<160>();
         softmax_warps<D, 2>(p, smem, misc, warp, lane);
     }
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 2) ptx::tmem_dealloc(misc->tmem_base, kTmemCols);
+    if (warp == 6) ptx::tmem_dealloc(misc->tmem_base, kTmemCols);
 #ifdef CP_TC_PROF
     if (threadIdx.x == 0) { misc->lane[0].prof[15] = (unsigned long long)(clock64() - t_start__); misc->lane[0].prof[13] -= (unsigned long long)t_start__; }
     __syncthreads();

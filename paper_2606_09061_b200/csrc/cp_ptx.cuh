@@ -218,9 +218,13 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {
 }
 
 __device__ __forceinline__ float ex2(float x) {
+#ifdef DL_X_NOEXP
+    return x * 0.001f;          // timing experiment only
+#else
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
+#endif
 }
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;
