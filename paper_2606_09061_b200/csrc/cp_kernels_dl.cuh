@@ -11,8 +11,8 @@
 // Each lane owns a TMA producer warp, an MMA issuer warp, four softmax warps, a K/V tile ring in
 // shared memory, its TMEM columns and its mbarriers; the lanes share nothing but the SM.
 //
-//   warpgroups 0-1: warps 0-2 TMA producers T, warps 3-5 TMA producers S, warp 6 MMA T,
-//                   warp 7 MMA S                                                    (48 regs)
+//   warpgroups 0-1: warps 0-2 TMA producers T, warps 3-4 TMA producers S, warps 5-6 MMA T (score
+//                   blocks / PV blocks), warp 7 MMA S                               (56 regs)
 //   warpgroup 2:    softmax T (thread <-> Q-tile row; also the decode items lane T runs once the
 //                   tile list is exhausted: thread <-> key)                         (232 regs)
 //   warpgroup 3:    softmax S (thread <-> key of the tile)                         (160 regs)
@@ -39,9 +39,9 @@ namespace dl {
 
 constexpr int kThreads = 512;
 constexpr int kStagesT = 3, kStagesS = 3, kMaxStages = 4;
-constexpr int kProdT = 3, kProdS = 3;         // TMA producer warps per lane (kProdT + kProdS + 2 MMA warps = 8 warps)
+constexpr int kProdT = 3, kProdS = 2;         // TMA producer warps per lane (kProdT + kProdS + 3 MMA warps = 8 warps)
 // a producer waiting for slot reuse may be at most one phase behind only if kProd <= kStages
-static_assert(kProdT <= kStagesT && kProdS <= kStagesS && kProdT + kProdS == 6, "producer / stage configuration");
+static_assert(kProdT <= kStagesT && kProdS <= kStagesS && kProdT + kProdS == 5, "producer / stage configuration");
 constexpr int kItemRing = 2;
 constexpr int kTmemCols = 512;
 // TMEM columns.  Lane T: S0, S1 (fp32 scores, P aliased over their first 64 columns), O, Q.
@@ -85,6 +85,7 @@ struct LaneState {              // one per lane, in the misc region
     uint64_t s_full[2];
     uint64_t p_full[2][2];      // [set][tile parity]: a waiter can never be two phases behind
     uint64_t pv_done[2];        // PV of tile gt completes on pv_done[gt & 1]
+    uint64_t pv_issued[2];      // lane T, tile kind: the PV issuer has put PV(t) into the pipe (per tile parity)
     uint64_t item_full[kItemRing];
     uint64_t item_empty[kItemRing];
     WorkItem items[kItemRing];  // published by the lane's producer; kind < 0 = no more work
@@ -115,6 +116,13 @@ struct Params {
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
     __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
     return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// One arrival per warp (after all its lanes are done) instead of 32: 128 single-word smem atomics
+// per barrier phase were a measurable part of every tile's critical path.
+__device__ __forceinline__ void warp_arrive(uint64_t* bar) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) ptx::mbar_arrive(bar);
 }
 
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
@@ -209,10 +217,16 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             const uint32_t slot = ld % kStages;
             { DL_T0; ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1); DL_ACC(8); }
             const bool leader = ptx::elect_one();
+#ifdef DL_X_NOTMA
+            if (leader) ptx::mbar_arrive(&ls->kv_full[slot]);
+            uint8_t* dst = kv_base + slot * L::kSlotBytes;
+            for (int j = 0; j < 0; ++j) {
+#else
             if (leader) ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u);
             uint8_t* dst = kv_base + slot * L::kSlotBytes;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
+#endif
                 const int pg = __shfl_sync(0xffffffffu, cur, (tile & 3) * 8 + j);
                 if (j < n_pages) {
                     const int slab = (pg * 2 + is_v) * p.sh.Hkv + kv_head;
@@ -226,32 +240,56 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
 }
 
 // ------------------------------------------------------------------------------------------
-// MMA issuer warp of a lane (tcgen05.mma is issued by one elected thread; the warp stays
-// convergent so descriptors live in uniform registers)
+// MMA issuer warps (tcgen05.mma is issued by one elected thread; the warp stays convergent so
+// descriptors live in uniform registers).
+//
+// The tensor pipe queues only a few instructions, and the serial work of an issuing thread between
+// two 8-instruction blocks (two or three mbarrier waits at ~90 cycles each, fences, descriptor
+// setup) left the pipe idle for about as long as a block runs.  Lane T therefore has TWO issuers
+// for chunk tiles: ROLE 1 issues the score blocks QK(t), ROLE 2 the PV(t) blocks; each does its
+// waiting while the other's block executes.  The only ordering the pipe needs between them is
+// "PV(t-2) before QK(t)" (QK(t) overwrites the S/P buffer PV(t-2) reads): ROLE 2 arrives on
+// pv_issued after issuing PV(t), ROLE 1 waits for it before QK(t+2).  Swap-kind items (lane S, and
+// lane T after its tile list is exhausted) are HBM-bound and keep a single issuer (ROLE 0 / ROLE 1).
 // ------------------------------------------------------------------------------------------
-template <int D, int LANE>
+template <int D, int LANE, int ROLE>
 __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
-                                         uint32_t& cons_cnt, uint32_t& gt, uint32_t (&gp)[2], uint32_t (&ic)[2]) {
+                                         uint32_t& ld_base, uint32_t& gt, uint32_t& gp, uint32_t (&ic)[2], uint32_t& gpt) {
     using L = Layout<D>;
     constexpr int kStages = LANE == 0 ? kStagesT : kStagesS;
     const int n_tiles = (__shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0) + kKeyTile - 1) / kKeyTile;
     const bool swap = LANE == 1 || __shfl_sync(0xffffffffu, it.kind, 0) == kKindSwap;
+    const bool all = ROLE == 0 || swap;        // this warp issues both kinds of block
+    if (ROLE == 2 && swap) {                   // not ours: stay in step
+        gt += n_tiles;
+        ld_base += 2 * n_tiles;
+        return;
+    }
+    const bool do_qk = all || ROLE == 1, do_pv = all || ROLE == 2;
     const uint32_t small = smem_base + L::kOffSmall[LANE], kv_base = smem_base + L::kOffKv[LANE];
     // tile kind: S = Q K^T (A = Q in TMEM, M 128 rows, N 128 keys); O += P V (A = P in TMEM, V MN-major B)
     // swap kind: S^T = K Q^T (M 128 keys, N 16);   O^T += V^T P^T (M 128 = D, N 16, V^T is MN-major A)
     const uint32_t idesc_qk = swap ? ptx::umma_idesc_bf16(128, 16, false, false) : ptx::umma_idesc_bf16(128, 128, false, false);
     const uint32_t idesc_pv = swap ? ptx::umma_idesc_bf16(128, 16, true, false) : ptx::umma_idesc_bf16(128, D, false, true);
     const uint32_t small_half = 2048;          // 16 rows x 128 B (Q^T / P^T halves in the swap kind)
-
     const int set = swap ? 1 : 0;              // barrier set and phase counters of this item kind
-    { DL_T0; ptx::mbar_wait(&ls->q_full[set], ic[set] & 1); DL_ACC(7); }
-    ptx::tc_fence_after();
+    const uint32_t g0 = gt, t0 = gpt;          // global tile counter / tile-kind tile counter at item start
+
+    if (do_qk) {
+        DL_T0;
+        ptx::mbar_wait(&ls->q_full[set], ic[set] & 1);
+        DL_ACC(7);
+        ptx::tc_fence_after();
+    }
     ++ic[set];
 
-    auto issue_qk = [&](uint32_t g) {          // g: global tile counter of the tile being scored
-        const uint32_t slot = cons_cnt % kStages, buf = g & 1;
+    // load order of the producers = consumption order: K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1)
+    auto issue_qk = [&](int t) {
+        const uint32_t ld = ld_base + (t == 0 ? 0 : 2 * t - 1);
+        const uint32_t slot = ld % kStages, buf = (g0 + t) & 1;
         DL_T0;
-        ptx::mbar_wait(&ls->kv_full[slot], (cons_cnt / kStages) & 1);
+        if (!all && t >= 2) ptx::mbar_wait(&ls->pv_issued[(t0 + t) & 1], ((t0 + t - 2) >> 1) & 1);   // PV(t-2) is in the pipe
+        ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
         DL_ACC(4);
         ptx::tc_fence_after();
         const uint32_t k_tile = kv_base + slot * L::kSlotBytes;
@@ -273,60 +311,58 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
         }
         __syncwarp();
         DL_ACC(11);
-        ++cons_cnt;
     };
-    auto issue_pv = [&](bool first) {
-        const uint32_t buf = gt & 1;
+    auto issue_pv = [&](int t) {
+        const uint32_t ld = ld_base + (t == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * t + 2);
+        const uint32_t slot = ld % kStages, buf = (g0 + t) & 1;
         DL_T0;
-        ptx::mbar_wait(&ls->p_full[set][gp[set] & 1], (gp[set] >> 1) & 1);
+        ptx::mbar_wait(&ls->p_full[set][gp & 1], (gp >> 1) & 1);
         DL_ACC(5);
-        ++gp[set];
-        const uint32_t slot = cons_cnt % kStages;
-        ptx::mbar_wait(&ls->kv_full[slot], (cons_cnt / kStages) & 1);
+        ++gp;
+        ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
         DL_ACC(6);
         ptx::tc_fence_after();
         const uint32_t v_tile = kv_base + slot * L::kSlotBytes;
         const uint32_t d_tmem = tmem + col_o(LANE);
         if (ptx::elect_one()) {
 #pragma unroll
-#ifdef DL_X_NOPV
-            for (int ks = 0; ks < 0; ++ks) {
-#else
             for (int ks = 0; ks < kKeyTile / 16; ++ks) {
-#endif
                 // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
                 const uint64_t v_desc = ptx::umma_desc_sw128(v_tile + ks * L::kPageBytes, 1024, L::kGroupBytes);
                 if (LANE == 0 && !swap) {
-                    umma_ts(d_tmem, tmem + col_s(0, buf) + ks * 8, v_desc, idesc_pv, !first || ks > 0);
+                    umma_ts(d_tmem, tmem + col_s(0, buf) + ks * 8, v_desc, idesc_pv, t > 0 || ks > 0);
                 } else {
                     const uint32_t poff = 4096 + buf * 4096 + (ks >> 2) * small_half + (ks & 3) * 32;   // P^T is double buffered
-                    ptx::umma_ss(d_tmem, v_desc, ptx::umma_desc_sw128(small + poff, 16, 1024), idesc_pv, !first || ks > 0);
+                    ptx::umma_ss(d_tmem, v_desc, ptx::umma_desc_sw128(small + poff, 16, 1024), idesc_pv, t > 0 || ks > 0);
                 }
             }
             ptx::umma_commit(&ls->kv_empty[slot]);
             ptx::umma_commit(&ls->pv_done[buf]);
+            if (!all) ptx::mbar_arrive(&ls->pv_issued[(t0 + t) & 1]);
         }
         __syncwarp();
         DL_ACC(12);
-        ++cons_cnt;
-        ++gt;
     };
 
-    // QK(k+1) is issued before PV(k) so the softmax of tile k overlaps the next score MMA.  p_full is
-    // indexed by tile parity (per item kind): the softmax of tile k+2 needs QK(k+2), which is issued
-    // only after p_full of tile k was observed here, so a wait can never alias onto a later phase.
-    issue_qk(gt);
-    for (int k = 0; k < n_tiles; ++k) {
-        if (k + 1 < n_tiles) issue_qk(gt + 1);
-        issue_pv(k == 0);
+    // QK(t+1) is issued before PV(t) so the softmax of tile t overlaps the next score MMA.  p_full is
+    // indexed by tile parity (per item kind): the softmax of tile t+2 needs QK(t+2), which is issued
+    // only after PV(t) was issued, i.e. after p_full of tile t was observed, so no wait can alias onto
+    // a later phase; the same argument covers pv_issued.
+    if (do_qk) issue_qk(0);
+    for (int t = 0; t < n_tiles; ++t) {
+        if (do_qk && t + 1 < n_tiles) issue_qk(t + 1);
+        if (do_pv) issue_pv(t);
     }
+    gt += n_tiles;
+    ld_base += 2 * n_tiles;
+    if (!swap) gpt += n_tiles;
 }
 
-template <int D, int LANE>
+template <int D, int LANE, int ROLE>
 __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lane) {
     LaneState* ls = &misc->lane[LANE];
     const uint32_t tmem = misc->tmem_base;
-    uint32_t cons_cnt = 0, gt = 0, item_cnt = 0, gp[2] = {0, 0}, ic[2] = {0, 0};
+    uint32_t ld_base = 0, gt = 0, item_cnt = 0, gp = 0, gpt = 0, ic[2] = {0, 0};
     for (;;) {
         const uint32_t islot = item_cnt % kItemRing;
         ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1);
@@ -334,7 +370,7 @@ __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lan
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&ls->item_empty[islot]);
         if (it.kind < 0) break;
-        mma_item<D, LANE>(it, smem_base, ls, tmem, cons_cnt, gt, gp, ic);
+        mma_item<D, LANE, ROLE>(it, smem_base, ls, tmem, ld_base, gt, gp, ic, gpt);
         ++item_cnt;
     }
 }
@@ -377,7 +413,7 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         }
         ptx::tmem_wait_st();
         ptx::tc_fence_before();
-        ptx::mbar_arrive(&ls->q_full[0]);
+        warp_arrive(&ls->q_full[0]);
     }
     DL_ACC(9);
 
@@ -391,10 +427,21 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         ptx::mbar_wait(&ls->s_full[buf], (gt >> 1) & 1);
         DL_ACC(0);
         ptx::tc_fence_after();
+#ifdef DL_X_NOTMEM
+        { l += 1.f; ptx::tc_fence_before(); warp_arrive(&ls->p_full[0][gp & 1]); ++gt; ++gp; continue; }
+#endif
         uint32_t sr[128];
 #pragma unroll
         for (int c = 0; c < 4; ++c) ptx::tmem_ld32(t_s + c * 32, sr + c * 32);
         ptx::tmem_wait_ld();
+#ifdef DL_X_NOSOFTMAX
+        { uint32_t pk[16];
+#pragma unroll
+          for (int j = 0; j < 16; ++j) pk[j] = 0x3c003c00u ^ (sr[j] & 1u);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) ptx::tmem_st16(t_s + c * 16, pk);
+          l += 1.f; ptx::tmem_wait_st(); ptx::tc_fence_before(); warp_arrive(&ls->p_full[0][gp & 1]); ++gt; ++gp; continue; }
+#endif
         const int nvalid = max(0, min(kKeyTile, limit - ts));
         float mx[8];                                    // 8 independent max chains
 #pragma unroll
@@ -456,7 +503,7 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         }
         ptx::tmem_wait_st();
         ptx::tc_fence_before();
-        ptx::mbar_arrive(&ls->p_full[0][gp & 1]);
+        warp_arrive(&ls->p_full[0][gp & 1]);
         DL_ACC(1);
         ++gt;
         ++gp;
@@ -521,7 +568,7 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
         *reinterpret_cast<uint4*>(small + (c >> 3) * 2048 + r * 128 + (((c & 7) ^ (r & 7)) << 4)) = v;
     }
     ptx::fence_proxy_async_smem();
-    ptx::mbar_arrive(&ls->q_full[1]);
+    warp_arrive(&ls->q_full[1]);
 
     float m_ref[RC], l_part[RC];
     int limit[RC];
@@ -593,7 +640,7 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
         ptx::fence_proxy_async_smem();
 #endif
         ptx::tc_fence_before();
-        ptx::mbar_arrive(&ls->p_full[1][gp & 1]);
+        warp_arrive(&ls->p_full[1][gp & 1]);
         ++gt;
         ++gp;
     }
@@ -646,7 +693,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
         const uint32_t islot = item_cnt % kItemRing;
         { DL_T0; ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1); DL_ACC(10); }
         const WorkItem it = ls->items[islot];
-        ptx::mbar_arrive(&ls->item_empty[islot]);
+        warp_arrive(&ls->item_empty[islot]);
         if (it.kind < 0) break;
         if (ROLE == 2 || it.kind == kKindSwap) {
             if constexpr (D == 128) {
@@ -678,16 +725,17 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         for (int ln = 0; ln < 2; ++ln) {
             LaneState* ls = &misc->lane[ln];
             for (int i = 0; i < kMaxStages; ++i) { ptx::mbar_init(&ls->kv_full[i], 1); ptx::mbar_init(&ls->kv_empty[i], 1); }
-            ptx::mbar_init(&ls->q_full[0], 128);
-            ptx::mbar_init(&ls->q_full[1], 128);
+            ptx::mbar_init(&ls->q_full[0], 4);
+            ptx::mbar_init(&ls->q_full[1], 4);
             for (int i = 0; i < 2; ++i) {
                 ptx::mbar_init(&ls->s_full[i], 1);
-                ptx::mbar_init(&ls->p_full[0][i], 128);
-                ptx::mbar_init(&ls->p_full[1][i], 128);
+                ptx::mbar_init(&ls->p_full[0][i], 4);
+                ptx::mbar_init(&ls->p_full[1][i], 4);
                 ptx::mbar_init(&ls->pv_done[i], 1);
+                ptx::mbar_init(&ls->pv_issued[i], 1);
             }
-            // readers of the item ring: the lane's 128 softmax threads, its MMA warp, its other producers
-            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], 128 + 1 + (ln == 0 ? kProdT : kProdS) - 1); }
+            // readers of the item ring (one arrival per warp): the lane's 4 softmax warps, its MMA warp(s), its other producers
+            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], 4 + (ln == 0 ? 2 + kProdT - 1 : 1 + kProdS - 1)); }
         }
         ptx::fence_barrier_init();
         ptx::prefetch_tmap(&tmap);
@@ -709,11 +757,12 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     // launch allocation: 128 registers per thread.  The two producer / MMA warpgroups give most of
     // their share to the tile softmax (a 128-column score row in registers) and the decode softmax.
     if (warp < 8) {
-        reg_dec<48>();
+        reg_dec<56>();
         if (warp < kProdT) producer<D, 0>(p, &tmap, smem, &misc->lane[0], lane, warp);
         else if (warp < kProdT + kProdS) producer<D, 1>(p, &tmap, smem, &misc->lane[1], lane, warp - kProdT);
-        else if (warp == 6) mma_warp<D, 0>(ptx::smem_u32(smem), misc, lane);
-        else mma_warp<D, 1>(ptx::smem_u32(smem), misc, lane);
+        else if (warp == 5) mma_warp<D, 0, 1>(ptx::smem_u32(smem), misc, lane);      // lane T: score blocks (and swap items)
+        else if (warp == 6) mma_warp<D, 0, 2>(ptx::smem_u32(smem), misc, lane);      // lane T: PV blocks
+        else mma_warp<D, 1, 0>(ptx::smem_u32(smem), misc, lane);                     // lane S
     } else if (warp < 12) {
         reg_inc<232>();
         softmax_warps<D, 0>(p, smem, misc, warp, lane);
