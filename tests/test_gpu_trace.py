@@ -103,3 +103,42 @@ def test_full_config5_trace():
         json.dump(report, f)
     assert report["e2e_s"]["finished"] == 1000
     assert n == len(log) and digest == report["schedule_sha256"]
+
+
+@pytest.mark.skipif(os.environ.get("CP_FULL_TRACE") != "1", reason="set CP_FULL_TRACE=1 (minutes, 40 GiB pool)")
+def test_lprs_apc_trace_with_trained_predictor():
+    """harvest cp_latency_table, train the Table-7 MLP, then run configs[4]
+    (compressed arrivals) under token budget / LPRS / LPRS+APC with that predictor; every schedule
+    must still equal the reference scheduler's replay (same predictor data on both sides)."""
+    from paper_2606_09061_b200 import predictor as pr
+    build.build()
+    raw, us = pr.harvest(int(os.environ.get("CP_HARVEST", "3000")), seed=0)
+    rep, lin, mlp = pr.train_and_report(raw, us, seed=0, epochs=int(os.environ.get("CP_EPOCHS", "300")))
+    X = pr.features16(raw)
+    full = X[:, 12] >= 2000
+    t_star = float(np.median(us[full]))                     # per-layer us of a typical full-budget round
+    rate = float(os.environ.get("CP_TRACE_RATE", "64"))
+    trace = wl.make_trace(1000, rate_per_s=rate, seed=0)
+    kind, w, mu, inv = pr.export_mlp(mlp)
+    base = dict(alpha=100.0, beta=-1.0, B_max=2048, S_max=1024, num_blocks=20480, block_size=16,
+                page_mb=2 * 8 * 16 * 128 * 2 * 32 / 2**20)
+    lprs = dict(base, mode=rs.MODE_LPRS, Delta=64, T_star=t_star, lambda_u=1.0, lambda_o=2.0, C_max=4, L_min=64,
+                pred_kind=kind, pred_weights=w, feat_mu=mu, feat_inv_sigma=inv)
+    out = {"predictor": rep, "T_star_us_per_layer": t_star, "arrival_rate_per_s": rate, "runs": {}}
+    for name, kw in [("token_budget", base), ("lprs", lprs), ("lprs_apc", dict(lprs, apc=True))]:
+        report, log = trace_run.run_trace(trace, sched_kw=kw)
+        digest, n = replay_reference(trace, log, **kw)
+        assert n == len(log) and digest == report["schedule_sha256"], name
+        assert report["e2e_s"]["finished"] == 1000
+        it = np.asarray(log, np.float64) / 32.0            # per-layer us of every iteration
+        mixed = report["iteration_us_by_class"]["mixed"]
+        report["per_layer_us"] = {"mean": float(it.mean()), "p95": float(np.percentile(it, 95)), "max": float(it.max()),
+                                  "frac_over_T_star": float((it > t_star).mean())}
+        report["mixed_iterations"] = mixed["iterations"]
+        report.pop("sched", None)
+        out["runs"][name] = report
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/lprs_report.json", "w") as f:
+        json.dump(out, f)
+    # latency control: LPRS keeps more iterations under the target than plain token-budget chunking
+    assert out["runs"]["lprs"]["per_layer_us"]["frac_over_T_star"] <= out["runs"]["token_budget"]["per_layer_us"]["frac_over_T_star"]
