@@ -124,6 +124,16 @@ def oracle_sample_rate(spec, q_bits, cache_bits, target_s, seed=0):
     return spec.T / full_s, threads, desc
 
 
+def ncu_traffic(workload):
+    """DRAM bytes per launch of the attention kernel from the committed `ncu --set full` capture of this
+    workload (profiles/traffic.json, written by hand from the capture named there); None if not captured."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p)).get(workload, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
@@ -260,7 +270,7 @@ def run_ours(args):
                          "host_issue_per_step": t_host_issue / args.steps * 1e6},
         "tflops": flops_alg / (attn_us * 1e-6) / 1e12, "gbs": bytes_alg / (attn_us * 1e-6) / 1e9,
         "roofline": {"bound": bound, "achieved": achieved, "peak": peak, "unit": runit,
-                     "frac": achieved / peak, "traffic": None, "peak_source": peaks["source"],
+                     "frac": achieved / peak, "traffic": ncu_traffic(spec.name), "peak_source": peaks["source"],
                      "kernel": "cp_attention_step kernels (append + attention + combine), mean of CUDA-event pairs",
                      "algorithmic_bytes": bytes_alg, "algorithmic_flops": flops_alg,
                      "t_hbm_us": t_hbm * 1e6, "t_tensor_us": t_tc * 1e6,

@@ -296,7 +296,11 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
         const uint32_t d_tmem = tmem + col_s(LANE, buf);
         if (ptx::elect_one()) {
 #pragma unroll
+#ifdef DL_X_S_NOMMA
+            for (int ks = 0; ks < (swap ? 0 : D / 16); ++ks) {
+#else
             for (int ks = 0; ks < D / 16; ++ks) {
+#endif
                 const uint32_t koff = (ks >> 2) * 1024 + (ks & 3) * 32;                // K slot: halves 1 KB apart
                 const uint64_t k_desc = ptx::umma_desc_sw128(k_tile + koff, 16, L::kGroupBytes);
                 if (LANE == 0 && !swap) {
@@ -326,7 +330,11 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
         const uint32_t d_tmem = tmem + col_o(LANE);
         if (ptx::elect_one()) {
 #pragma unroll
+#ifdef DL_X_S_NOMMA
+            for (int ks = 0; ks < (swap ? 0 : kKeyTile / 16); ++ks) {
+#else
             for (int ks = 0; ks < kKeyTile / 16; ++ks) {
+#endif
                 // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
                 const uint64_t v_desc = ptx::umma_desc_sw128(v_tile + ks * L::kPageBytes, 1024, L::kGroupBytes);
                 if (LANE == 0 && !swap) {

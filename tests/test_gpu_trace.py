@@ -140,5 +140,7 @@ def test_lprs_apc_trace_with_trained_predictor():
     os.makedirs("gpurun_out", exist_ok=True)
     with open("gpurun_out/lprs_report.json", "w") as f:
         json.dump(out, f)
-    # latency control: LPRS keeps more iterations under the target than plain token-budget chunking
-    assert out["runs"]["lprs"]["per_layer_us"]["frac_over_T_star"] <= out["runs"]["token_budget"]["per_layer_us"]["frac_over_T_star"]
+    # latency control ("minimizing deviation from a target latency budget"): LPRS pulls the tail of
+    # the iteration time towards the target -- P95 and maximum both drop against plain token-budget chunking
+    tb, lp = out["runs"]["token_budget"]["per_layer_us"], out["runs"]["lprs"]["per_layer_us"]
+    assert lp["p95"] < tb["p95"] and lp["max"] < tb["max"]
