@@ -85,7 +85,12 @@ struct LaneState {              // one per lane, in the misc region
     uint64_t s_full[2];
     uint64_t p_full[2][2];      // [set][tile parity]: a waiter can never be two phases behind
     uint64_t pv_done[2];        // PV of tile gt completes on pv_done[gt & 1]
-    uint64_t pv_issued[2];      // lane T, tile kind: the PV issuer has put PV(t) into the pipe (per tile parity)
+    // lane T, tile kind: a 128-key tile is scored as two 64-key half-tiles; FOUR 64-column S buffers
+    // (index = half-tile counter & 3) keep four softmax <-> MMA round trips in flight
+    uint64_t ts_full[4];        // scores of half-tile j are in S buffer j & 3
+    uint64_t tp_full[4];        // P of half-tile j is in place
+    uint64_t tpv_done[4];       // PV of half-tile j has completed
+    uint64_t pv_issued[4];      // the PV issuer has put PV(j) into the pipe
     uint64_t item_full[kItemRing];
     uint64_t item_empty[kItemRing];
     WorkItem items[kItemRing];  // published by the lane's producer; kind < 0 = no more work
@@ -252,6 +257,84 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
 // pv_issued after issuing PV(t), ROLE 1 waits for it before QK(t+2).  Swap-kind items (lane S, and
 // lane T after its tile list is exhausted) are HBM-bound and keep a single issuer (ROLE 0 / ROLE 1).
 // ------------------------------------------------------------------------------------------
+// Lane T, tile kind.  The item's key range is scored in 64-key half-tiles j = 0 .. nh-1 (tile j >> 1,
+// half j & 1); half-tile j uses S buffer (gh0 + j) & 3.  ROLE 1 issues QK(j) (N = 64), ROLE 2 issues
+// PV(j) (4 K-steps of 16 keys).  A K/V ring slot still holds a whole 128-key tile: it is waited for at
+// its first half and released (tcgen05.commit -> kv_empty) after its last.
+template <int D, int ROLE>
+__device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
+                                              uint32_t& ld_base, uint32_t& gh, uint32_t (&ic)[2]) {
+    using L = Layout<D>;
+    constexpr int kStages = kStagesT;
+    const int n_keys = __shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0);
+    const int n_tiles = (n_keys + kKeyTile - 1) / kKeyTile, nh = (n_keys + 63) / 64;
+    const uint32_t kv_base = smem_base + L::kOffKv[0];
+    const uint32_t idesc_qk = ptx::umma_idesc_bf16(128, 64, false, false);
+    const uint32_t idesc_pv = ptx::umma_idesc_bf16(128, D, false, true);
+    const uint32_t gh0 = gh;
+    if (ROLE == 1) {
+        DL_T0;
+        ptx::mbar_wait(&ls->q_full[0], ic[0] & 1);
+        DL_ACC(7);
+        ptx::tc_fence_after();
+    }
+    ++ic[0];
+    for (int j = 0; j < nh; ++j) {
+        const int t = j >> 1, h = j & 1;
+        const uint32_t g = gh0 + j, buf = g & 3;
+        const bool last_of_slot = h == 1 || j == nh - 1;
+        if (ROLE == 1) {
+            // load order of the producers: K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1)
+            const uint32_t ld = ld_base + (t == 0 ? 0 : 2 * t - 1);
+            const uint32_t slot = ld % kStages;
+            DL_T0;
+            if (j >= 4) ptx::mbar_wait(&ls->pv_issued[buf], ((g - 4) >> 2) & 1);      // PV(j-4) (same S buffer) is in the pipe
+            if (h == 0) ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+            DL_ACC(4);
+            ptx::tc_fence_after();
+            const uint32_t k_half = kv_base + slot * L::kSlotBytes + h * 8 * L::kGroupBytes;   // rows 64 h .. 64 h + 63
+            const uint32_t d_tmem = tmem + buf * 64;
+            if (ptx::elect_one()) {
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    const uint32_t koff = (ks >> 2) * 1024 + (ks & 3) * 32;            // K slot: halves of D 1 KB apart
+                    umma_ts(d_tmem, tmem + kColQ + ks * 8, ptx::umma_desc_sw128(k_half + koff, 16, L::kGroupBytes), idesc_qk, ks > 0);
+                }
+                if (last_of_slot) ptx::umma_commit(&ls->kv_empty[slot]);
+                ptx::umma_commit(&ls->ts_full[buf]);
+            }
+            __syncwarp();
+            DL_ACC(11);
+        } else {
+            const uint32_t ld = ld_base + (t == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * t + 2);
+            const uint32_t slot = ld % kStages;
+            DL_T0;
+            ptx::mbar_wait(&ls->tp_full[buf], (g >> 2) & 1);
+            DL_ACC(5);
+            if (h == 0) ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+            DL_ACC(6);
+            ptx::tc_fence_after();
+            const uint32_t v_half = kv_base + slot * L::kSlotBytes + h * 4 * L::kPageBytes;     // keys 64 h .. 64 h + 63
+            const uint32_t d_tmem = tmem + col_o(0);
+            if (ptx::elect_one()) {
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) {
+                    // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
+                    umma_ts(d_tmem, tmem + buf * 64 + ks * 8, ptx::umma_desc_sw128(v_half + ks * L::kPageBytes, 1024, L::kGroupBytes),
+                            idesc_pv, j > 0 || ks > 0);
+                }
+                if (last_of_slot) ptx::umma_commit(&ls->kv_empty[slot]);
+                ptx::umma_commit(&ls->tpv_done[buf]);
+                ptx::mbar_arrive(&ls->pv_issued[buf]);
+            }
+            __syncwarp();
+            DL_ACC(12);
+        }
+    }
+    gh += nh;
+    ld_base += 2 * n_tiles;
+}
+
 template <int D, int LANE, int ROLE>
 __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
                                          uint32_t& ld_base, uint32_t& gt, uint32_t& gp, uint32_t (&ic)[2], uint32_t& gpt) {
@@ -260,7 +343,11 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
     const int n_tiles = (__shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0) + kKeyTile - 1) / kKeyTile;
     const bool swap = LANE == 1 || __shfl_sync(0xffffffffu, it.kind, 0) == kKindSwap;
     const bool all = ROLE == 0 || swap;        // this warp issues both kinds of block
-    if (ROLE == 2 && swap) {                   // not ours: stay in step
+    if (!swap) {
+        if constexpr (LANE == 0 && ROLE != 0) mma_tile_item<D, ROLE>(it, smem_base, ls, tmem, ld_base, gpt, ic);
+        return;
+    }
+    if (ROLE == 2) {                           // swap item on lane T: ROLE 1 issues it; stay in step
         gt += n_tiles;
         ld_base += 2 * n_tiles;
         return;
@@ -363,7 +450,6 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
     }
     gt += n_tiles;
     ld_base += 2 * n_tiles;
-    if (!swap) gpt += n_tiles;
 }
 
 template <int D, int LANE, int ROLE>
@@ -392,7 +478,7 @@ __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lan
 // ------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p, LaneState* ls, uint32_t tmem,
-                                             uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base) {
+                                             uint32_t& gh, int row, uint32_t lane_base) {
     const Shape& sh = p.sh;
     const int G = sh.G;
     const int R = it.q_tokens * G;
@@ -427,42 +513,39 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
 
     const int limit = valid_row ? min(it.kv_end, ctx + it.q_start + row / G + 1) : 0;   // causal, diagonal inclusive
     float m_ref = -INFINITY, l = 0.f;
+    const int nh = (it.kv_end - it.kv_begin + 63) / 64;          // 64-key half-tiles, S buffer = gh & 3
 
-    for (int k = 0; k < n_tiles; ++k) {
-        const int ts = it.kv_begin + k * kKeyTile;
-        const uint32_t buf = gt & 1;
-        const uint32_t t_s = t_row + col_s(0, buf);
-        ptx::mbar_wait(&ls->s_full[buf], (gt >> 1) & 1);
+    for (int j = 0; j < nh; ++j) {
+        const int ts = it.kv_begin + j * 64;
+        const uint32_t buf = gh & 3;
+        const uint32_t t_s = t_row + buf * 64;
+        ptx::mbar_wait(&ls->ts_full[buf], (gh >> 2) & 1);
         DL_ACC(0);
         ptx::tc_fence_after();
 #ifdef DL_X_NOTMEM
-        { l += 1.f; ptx::tc_fence_before(); warp_arrive(&ls->p_full[0][gp & 1]); ++gt; ++gp; continue; }
+        { l += 1.f; ptx::tc_fence_before(); warp_arrive(&ls->tp_full[buf]); ++gh; continue; }
 #endif
-        uint32_t sr[128];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) ptx::tmem_ld32(t_s + c * 32, sr + c * 32);
+        uint32_t sr[64];
+        ptx::tmem_ld32(t_s, sr);
+        ptx::tmem_ld32(t_s + 32, sr + 32);
         ptx::tmem_wait_ld();
 #ifdef DL_X_NOSOFTMAX
-        { uint32_t pk[16];
+        { uint32_t pk[32];
 #pragma unroll
-          for (int j = 0; j < 16; ++j) pk[j] = 0x3c003c00u ^ (sr[j] & 1u);
-#pragma unroll
-          for (int c = 0; c < 4; ++c) ptx::tmem_st16(t_s + c * 16, pk);
-          l += 1.f; ptx::tmem_wait_st(); ptx::tc_fence_before(); warp_arrive(&ls->p_full[0][gp & 1]); ++gt; ++gp; continue; }
+          for (int i = 0; i < 32; ++i) pk[i] = 0x3c003c00u ^ (sr[i] & 1u);
+          ptx::tmem_st32(t_s, pk);
+          l += 1.f; ptx::tmem_wait_st(); ptx::tc_fence_before(); warp_arrive(&ls->tp_full[buf]); ++gh; continue; }
 #endif
-        const int nvalid = max(0, min(kKeyTile, limit - ts));
-        float mx[8];                                    // 8 independent max chains
+        const int nvalid = max(0, min(64, limit - ts));
+        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};      // independent max chains
+        if (nvalid == 64) {
 #pragma unroll
-        for (int i = 0; i < 8; ++i) mx[i] = -INFINITY;
-        if (nvalid == kKeyTile) {
-#pragma unroll
-            for (int j = 0; j < 128; ++j) mx[j & 7] = fmaxf(mx[j & 7], __uint_as_float(sr[j]));
+            for (int i = 0; i < 64; ++i) mx[i & 3] = fmaxf(mx[i & 3], __uint_as_float(sr[i]));
         } else {
 #pragma unroll
-            for (int j = 0; j < 128; ++j) mx[j & 7] = fmaxf(mx[j & 7], j < nvalid ? __uint_as_float(sr[j]) : -INFINITY);
+            for (int i = 0; i < 64; ++i) mx[i & 3] = fmaxf(mx[i & 3], i < nvalid ? __uint_as_float(sr[i]) : -INFINITY);
         }
-        float m_t = fmaxf(fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])), fmaxf(fmaxf(mx[4], mx[5]), fmaxf(mx[6], mx[7])));
-        m_t *= scale;                                   // scale > 0
+        const float m_t = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * scale;      // scale > 0
         float alpha = 1.f;
         bool rescale = false;
         if (m_t > m_ref + kRescaleThreshold) {          // also the first finite max (m_ref = -inf)
@@ -472,32 +555,28 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         }
         const float neg_m = (m_ref == -INFINITY) ? 0.f : -m_ref;
         float sm[4] = {0.f, 0.f, 0.f, 0.f};             // independent sum chains
+        uint32_t pk[32];                                // 64 scores -> 32 packed P columns
+        if (nvalid == 64) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {                   // 32 scores -> 16 packed P columns
-            uint32_t pk[16];
-            if (nvalid == kKeyTile) {
-#pragma unroll
-                for (int j = 0; j < 32; j += 2) {
-                    const float a = ptx::ex2(fmaf(__uint_as_float(sr[c * 32 + j]), scale, neg_m));
-                    const float b = ptx::ex2(fmaf(__uint_as_float(sr[c * 32 + j + 1]), scale, neg_m));
-                    sm[(j >> 1) & 3] += a + b;
-                    pk[j >> 1] = pack_bf16(a, b);
-                }
-            } else {
-#pragma unroll
-                for (int j = 0; j < 32; j += 2) {
-                    const int key = c * 32 + j;
-                    const float a = key < nvalid ? ptx::ex2(fmaf(__uint_as_float(sr[key]), scale, neg_m)) : 0.f;
-                    const float b = key + 1 < nvalid ? ptx::ex2(fmaf(__uint_as_float(sr[key + 1]), scale, neg_m)) : 0.f;
-                    sm[(j >> 1) & 3] += a + b;
-                    pk[j >> 1] = pack_bf16(a, b);
-                }
+            for (int i = 0; i < 64; i += 2) {
+                const float a = ptx::ex2(fmaf(__uint_as_float(sr[i]), scale, neg_m));
+                const float b = ptx::ex2(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m));
+                sm[(i >> 1) & 3] += a + b;
+                pk[i >> 1] = pack_bf16(a, b);
             }
-            ptx::tmem_st16(t_s + c * 16, pk);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 64; i += 2) {
+                const float a = i < nvalid ? ptx::ex2(fmaf(__uint_as_float(sr[i]), scale, neg_m)) : 0.f;
+                const float b = i + 1 < nvalid ? ptx::ex2(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m)) : 0.f;
+                sm[(i >> 1) & 3] += a + b;
+                pk[i >> 1] = pack_bf16(a, b);
+            }
         }
+        ptx::tmem_st32(t_s, pk);
         l = l * alpha + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
-        if (k > 0 && __any_sync(0xffffffffu, rescale)) {
-            ptx::mbar_wait(&ls->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);      // PV(k-1) done: O readable
+        if (j > 0 && __any_sync(0xffffffffu, rescale)) {
+            ptx::mbar_wait(&ls->tpv_done[(gh - 1) & 3], ((gh - 1) >> 2) & 1);      // PV(j-1) (and all before) done: O readable
             ptx::tc_fence_after();
 #pragma unroll 1
             for (int c = 0; c < D / 32; ++c) {
@@ -505,20 +584,19 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
                 ptx::tmem_ld32(t_row + col_o(0) + c * 32, o);
                 ptx::tmem_wait_ld();
 #pragma unroll
-                for (int j = 0; j < 32; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
                 ptx::tmem_st32(t_row + col_o(0) + c * 32, o);
             }
         }
         ptx::tmem_wait_st();
         ptx::tc_fence_before();
-        warp_arrive(&ls->p_full[0][gp & 1]);
+        warp_arrive(&ls->tp_full[buf]);
         DL_ACC(1);
-        ++gt;
-        ++gp;
+        ++gh;
     }
 
     // ---- epilogue: O row from TMEM (one load batch) -> out (bf16, normalised) or split workspace (fp32, unnormalised)
-    ptx::mbar_wait(&ls->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
+    ptx::mbar_wait(&ls->tpv_done[(gh - 1) & 3], ((gh - 1) >> 2) & 1);
     DL_ACC(2);
     ptx::tc_fence_after();
     const float inv = 1.f / l;
@@ -696,7 +774,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
     const uint32_t lane_base = (warp & 3) * 32;
     const int row = lane_base + lane;
     uint8_t* small = smem + L::kOffSmall[LANE];
-    uint32_t gt = 0, item_cnt = 0, gp_tile = 0, gp_swap = 0;
+    uint32_t gt = 0, item_cnt = 0, gh_tile = 0, gp_swap = 0;      // gt / gp_swap: swap-kind tiles; gh_tile: tile-kind half-tiles
     for (;;) {
         const uint32_t islot = item_cnt % kItemRing;
         { DL_T0; ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1); DL_ACC(10); }
@@ -711,7 +789,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
                 else softmax_swap<LANE, 16>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
             }
         } else {
-            if constexpr (ROLE == 0) softmax_tile<D>(it, p, ls, tmem, gt, gp_tile, row, lane_base);
+            if constexpr (ROLE == 0) softmax_tile<D>(it, p, ls, tmem, gh_tile, row, lane_base);
         }
         ++item_cnt;
     }
@@ -740,6 +818,11 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 ptx::mbar_init(&ls->p_full[0][i], 4);
                 ptx::mbar_init(&ls->p_full[1][i], 4);
                 ptx::mbar_init(&ls->pv_done[i], 1);
+            }
+            for (int i = 0; i < 4; ++i) {
+                ptx::mbar_init(&ls->ts_full[i], 1);
+                ptx::mbar_init(&ls->tp_full[i], 4);
+                ptx::mbar_init(&ls->tpv_done[i], 1);
                 ptx::mbar_init(&ls->pv_issued[i], 1);
             }
             // readers of the item ring (one arrival per warp): the lane's 4 softmax warps, its MMA warp(s), its other producers
