@@ -270,7 +270,7 @@ def run_ours(args):
                          "host_issue_per_step": t_host_issue / args.steps * 1e6},
         "tflops": flops_alg / (attn_us * 1e-6) / 1e12, "gbs": bytes_alg / (attn_us * 1e-6) / 1e9,
         "roofline": {"bound": bound, "achieved": achieved, "peak": peak, "unit": runit,
-                     "frac": achieved / peak, "traffic": ncu_traffic(spec.name), "peak_source": peaks["source"],
+                     "frac": achieved / peak, "traffic": ncu_traffic(spec.name) if args.variant == 0 else None, "peak_source": peaks["source"],
                      "kernel": "cp_attention_step kernels (append + attention + combine), mean of CUDA-event pairs",
                      "algorithmic_bytes": bytes_alg, "algorithmic_flops": flops_alg,
                      "t_hbm_us": t_hbm * 1e6, "t_tensor_us": t_tc * 1e6,

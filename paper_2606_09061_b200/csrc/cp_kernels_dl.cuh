@@ -19,7 +19,7 @@
 // (Measured alternatives, round 1: splitting a score tile over two softmax warpgroups, and
 // reading the score row in chunks, were no faster -- see DESIGN.md section 6.)
 //
-//   kKindTile   S[128 rows x 128 keys] = Q K^T with Q held in TMEM (A operand from TMEM, written
+//   kKindTile   S[128 rows x 64 keys] = Q K^T per half-tile, with Q held in TMEM (A operand from TMEM, written
 //               once per item with tcgen05.st), P written back over S in TMEM as bf16 and consumed
 //               as the A operand of O[128 x D] += P V.  Neither Q nor P touches shared memory, so
 //               the smem crossbar carries only the K/V tiles (TMA writes + one MMA read each).
@@ -44,7 +44,8 @@ constexpr int kProdT = 3, kProdS = 2;         // TMA producer warps per lane (kP
 static_assert(kProdT <= kStagesT && kProdS <= kStagesS && kProdT + kProdS == 5, "producer / stage configuration");
 constexpr int kItemRing = 2;
 constexpr int kTmemCols = 512;
-// TMEM columns.  Lane T: S0, S1 (fp32 scores, P aliased over their first 64 columns), O, Q.
+// TMEM columns.  Lane T: four 64-column S buffers at 0 / 64 / 128 / 192 (fp32 scores of a 64-key
+// half-tile, P aliased over their first 32 columns; the swap kind uses columns 0 and 128), O, Q.
 // Lane S: 16-column S^T0, S^T1, O^T.
 __host__ __device__ constexpr uint32_t col_s(int lane, uint32_t buf) { return lane == 0 ? buf * 128u : 448u + buf * 16u; }
 __host__ __device__ constexpr uint32_t col_o(int lane) { return lane == 0 ? 256u : 480u; }
