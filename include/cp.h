@@ -48,6 +48,9 @@ typedef struct cp_sched cp_sched;   /* opaque */
  *     kv_cache[layer][block][kv: 0 = K, 1 = V][kv_head][slot in 0..B-1][d in 0..D-1]
  * A (block, kv, head) slab is B*D*2 bytes contiguous (4 KiB at B 16, D 128); K and V
  * of a block are adjacent.  cp_attention_step takes the pointer to the LAYER's pool.
+ * Pages named by a block table must hold FINITE bf16 values in all their slots, written
+ * or not (zero-fill the pool once after allocating it): masked probabilities are exactly
+ * 0, but 0 x NaN in the tensor-core PV product would still be NaN.
  * ------------------------------------------------------------------------------- */
 typedef struct {
     int32_t num_q_heads;      /* Hq                                               */

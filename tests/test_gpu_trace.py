@@ -144,3 +144,26 @@ def test_lprs_apc_trace_with_trained_predictor():
     # the iteration time towards the target -- P95 and maximum both drop against plain token-budget chunking
     tb, lp = out["runs"]["token_budget"]["per_layer_us"], out["runs"]["lprs"]["per_layer_us"]
     assert lp["p95"] < tb["p95"] and lp["max"] < tb["max"]
+
+
+def test_apc_ablation_shape_trace_on_gpu():
+    """the APC ablation workload shape (49:1 short (30-50) : long (200-220)
+    prompts, bursty arrivals) -- many tiny chunks per iteration -- through the whole path with LPRS + APC on,
+    oracle parity on sampled iterations and schedule identity with the reference."""
+    build.build()
+    Hq, Hkv, D, B, layers = 32, 8, 128, 16, 2
+    trace = wl.make_apc_trace(300, seed=2, mean_gap_us=8.0)          # arrivals faster than iterations: the queue has depth
+    lin_w = [0.0] * 16
+    lin_w[11], lin_w[12], lin_w[14], lin_w[15] = 8.0, 0.02, 0.0004, 1e-6          # us per layer: bias, tokens, decode ctx, prefill interaction
+    kw = dict(alpha=100.0, beta=-1.0, B_max=96, S_max=64, mode=rs.MODE_LPRS, apc=True, Delta=8, T_star=11.0, C_max=2, L_min=16,
+              num_blocks=4096, block_size=B, pred_weights=lin_w)
+    stats = []
+    scale = float(np.float32(1.0) / np.sqrt(np.float32(D)))
+    hook = make_parity_hook(Hq, Hkv, D, B, layers, 25, 128, stats, scale)
+    report, log = trace_run.run_trace(trace, Hq=Hq, Hkv=Hkv, D=D, B=B, layers=layers, pages_per_layer=4096,
+                                      sched_kw=kw, seed=2, hook=hook)
+    assert report["e2e_s"]["finished"] == 300 and len(stats) >= 10
+    assert report["blocked_by_activity_cap"] + report["blocked_by_min_chunk"] > 0      # APC intervened (Table 10 counters)
+    kw_ref = dict(kw, page_mb=2 * Hkv * B * D * 2 * layers / 2**20)
+    digest, n = replay_reference(trace, log, **kw_ref)
+    assert n == len(log) and digest == report["schedule_sha256"]
