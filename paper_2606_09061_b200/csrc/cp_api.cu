@@ -73,6 +73,7 @@ struct cp_ctx {
     float feat[CP_NUM_RAW_FEATURES] = {0};
     float mem_stats[4] = {0, 0, 0, 0};
     int32_t n_prefill = 0, n_decode = 0;
+    int32_t combine_rows = 0;          // rows (token, head) that have split partials to merge
 
     // latency ring
     std::vector<TimedStep> ring;
@@ -202,7 +203,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     if (n_reqs > c->cfg.max_reqs) { cp_set_error("cp_build_batch: %d requests > max_reqs %d", n_reqs, c->cfg.max_reqs); return CP_ECAPACITY; }
 
     // ---- validate + totals ------------------------------------------------------------
-    int64_t T = 0, P = 0, total_tiles = 0;
+    int64_t T = 0, P = 0, total_tiles[2] = {0, 0};      // key tiles per item kind (tile, swap)
     float f_pf_tokens = 0, f_dec = 0, f_sum_ctx = 0, f_max_ctx = 0, f_pf_proc = 0, f_pf_proc_max = 0;
     int32_t n_prefill = 0, n_decode = 0;
     for (int j = 0; j < n_reqs; ++j) {
@@ -233,18 +234,33 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
             f_pf_proc_max = std::max(f_pf_proc_max, (float)r.ctx_off);
         }
         for (int q0 = 0; q0 < r.q_len; q0 += TQ) {
-            const int64_t lim = (int64_t)r.ctx_off + std::min(r.q_len, q0 + TQ);
-            total_tiles += (lim + kKeyTile - 1) / kKeyTile * sh.Hkv;
+            const int qt = std::min(TQ, r.q_len - q0);
+            const int64_t lim = (int64_t)r.ctx_off + q0 + qt;
+            const int kind = (c->use_tc && qt * G <= 16 && sh.D == 128) ? kKindSwap : kKindTile;
+            total_tiles[kind] += (lim + kKeyTile - 1) / kKeyTile * sh.Hkv;
         }
     }
     if (T > c->cfg.max_tokens) { cp_set_error("cp_build_batch: %lld tokens > max_tokens %d", (long long)T, c->cfg.max_tokens); return CP_ECAPACITY; }
     if (P > c->cfg.max_total_pages) { cp_set_error("cp_build_batch: %lld pages > max_total_pages %lld", (long long)P, (long long)c->cfg.max_total_pages); return CP_ECAPACITY; }
 
     // ---- plan: split long key ranges so the persistent grid stays balanced ---------------
-    // ~12 items per SM on average; an item is never longer than total / (12 * n_sm) tiles, so
-    // the LPT-ordered dynamic schedule ends with a short tail.
-    const int64_t per = (int64_t)c->n_sm * 12;
-    int chunk_tiles = (int)std::min<int64_t>(1 << 20, std::max<int64_t>(1, (total_tiles + per - 1) / per));
+    // An item is never longer than (total key tiles of the batch) / (n_sm * P), so the LPT-ordered
+    // dynamic schedule ends with a short tail.  Splitting a chunk tile is expensive (a 64 KiB fp32
+    // partial per split, a second pipeline fill, the combine pass), so tile-kind items are split only
+    // when LPT needs it (P = 1: no item above the mean load of an SM); decode items cost 2 KiB per
+    // split, and a decode-only batch should give each of the two lanes of an SM an item (P = 2).
+    // Measured on B200: P = 12 for both kinds cost 14 % on the chunks of
+    // configs[2] and 20 % on configs[1].
+    int per_sm[2] = {1, 2};
+    if (!c->use_dl) per_sm[0] = per_sm[1] = 12;
+    if (const char* e = getenv("CP_X_PT")) per_sm[0] = atoi(e);                   // experiments only
+    if (const char* e = getenv("CP_X_PS")) per_sm[1] = atoi(e);
+    int chunk_of[2];
+    for (int k = 0; k < 2; ++k) {
+        const int64_t total = total_tiles[0] + total_tiles[1];     // the lanes share the SMs: mean load of the whole batch
+        const int64_t per = (int64_t)c->n_sm * per_sm[k];
+        chunk_of[k] = (int)std::min<int64_t>(1 << 20, std::max<int64_t>(1, (total + per - 1) / per));
+    }
     int64_t partial_rows = 0;
     for (int attempt = 0;; ++attempt) {
         c->items.clear();
@@ -263,6 +279,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
                 const int q0 = qi * TQ, qt = std::min(TQ, r.q_len - q0), rows = qt * G;
                 const int lim = r.ctx_off + q0 + qt;                 // causal limit of the last row
                 const int n_tiles = (lim + kKeyTile - 1) / kKeyTile;
+                const int chunk_tiles = chunk_of[(c->use_tc && rows <= 16 && sh.D == 128) ? kKindSwap : kKindTile];
                 const int n_splits = (n_tiles + chunk_tiles - 1) / chunk_tiles;
                 c->plan[2 * qi] = n_splits;
                 c->plan[2 * qi + 1] = (n_tiles + n_splits - 1) / n_splits;
@@ -274,7 +291,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
                         partial_rows += (int64_t)n_splits * rows;
                         if (partial_rows > c->max_partial_rows || partial_rows > INT32_MAX ||
                             c->combines.size() >= c->max_combine) { overflow = true; break; }
-                        c->combines.push_back(CombineItem{(int32_t)(tok + q0), qt, g, n_splits, prow, {0, 0, 0}});
+                        c->combines.push_back(CombineItem{(int32_t)(tok + q0), qt, g, n_splits, prow, 0, {0, 0}});
                     }
                     c->plan_prow[(size_t)qi * sh.Hkv + g] = prow;
                 }
@@ -301,8 +318,9 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
             tok += r.q_len;
         }
         if (!overflow) break;
-        if (chunk_tiles >= (1 << 20)) { cp_set_error("cp_build_batch: work list does not fit the limits of cp_create"); return CP_ECAPACITY; }
-        chunk_tiles *= 2;                                            // coarser splits need less workspace
+        if (chunk_of[0] >= (1 << 20) && chunk_of[1] >= (1 << 20)) { cp_set_error("cp_build_batch: work list does not fit the limits of cp_create"); return CP_ECAPACITY; }
+        chunk_of[0] = std::min(1 << 20, chunk_of[0] * 2);            // coarser splits need less workspace
+        chunk_of[1] = std::min(1 << 20, chunk_of[1] * 2);
     }
 
     // ---- LPT order: bucket sort by descending number of key tiles.  The dual-lane kernel takes the
@@ -356,6 +374,11 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
         for (int i = 0; i < r.q_len; ++i) tr[cu[j] + i] = j;
     }
     std::memcpy(h + o_wk, c->sorted.data(), sizeof(WorkItem) * n_items);
+    {   // prefix sums of the groups' row counts: the combine kernel maps one warp to one row
+        int32_t rows = 0;
+        for (CombineItem& ci : c->combines) { ci.row_base = rows; rows += ci.q_tokens * G; }
+        c->combine_rows = rows;
+    }
     std::memcpy(h + o_cb, c->combines.data(), sizeof(CombineItem) * c->combines.size());
 
     if (off > 0) CP_CUDA(cudaMemcpyAsync(c->d_meta, h, off, cudaMemcpyHostToDevice, stream));
@@ -403,7 +426,7 @@ static int launch_simt(cp_ctx* c, const __nv_bfloat16* q, const __nv_bfloat16* c
         CP_CUDA(cudaGetLastError());
     }
     if (m.n_combine > 0) {
-        combine_kernel<D><<<dim3(m.n_combine, 32), 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
+        combine_kernel<D><<<(c->combine_rows + 3) / 4, 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
         CP_CUDA(cudaGetLastError());
     }
     return CP_OK;
@@ -476,7 +499,7 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
         c->info.grid_attn = grid;
     }
     if (m.n_combine > 0) {
-        combine_kernel<D><<<dim3(m.n_combine, 32), 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
+        combine_kernel<D><<<(c->combine_rows + 3) / 4, 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
         CP_CUDA(cudaGetLastError());
         ++*launches;
     }

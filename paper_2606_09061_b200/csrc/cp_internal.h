@@ -37,7 +37,8 @@ struct CombineItem {
     int32_t kv_head;
     int32_t n_splits;
     int32_t partial_row;   // split s occupies rows [partial_row + s*R, +R), R = q_tokens*G
-    int32_t pad[3];
+    int32_t row_base;      // sum of R over the preceding combine items (warp <-> row mapping)
+    int32_t pad[2];
 };
 static_assert(sizeof(CombineItem) == 32, "CombineItem is 32 bytes");
 

@@ -125,21 +125,28 @@ attn_simt_kernel(BatchMeta meta, Shape sh, const __nv_bfloat16* __restrict__ q,
 }
 
 // ---------------------------------------------------------------------------------
-// H5: out = sum_s w_s O_s / sum_s w_s l_s, w_s = 2^(m_s - max m).  One warp per row:
-// grid (n_combine, ceil(128 / 4)), warp w of block (i, y) merges row 4y + w of item i.  The
-// (m, l) pairs of up to 32 splits are read one per lane and the weights broadcast by shuffle, so
-// the O_s loads of a row are independent and issue back to back.
+// H5: out = sum_s w_s O_s / sum_s w_s l_s, w_s = 2^(m_s - max m).  One warp per (token, head) row
+// that has split partials: global warp gw finds its combine item by binary search over the items'
+// row_base prefix sums (a grid of one block per item x 32 row slots was dominated by the launch of
+// empty blocks).  The (m, l) pairs of up to 32 splits are read one per lane and the weights
+// broadcast by shuffle, so the O_s loads of a row are independent and issue back to back.
 // ---------------------------------------------------------------------------------
 template <int D>
 __global__ void __launch_bounds__(128)
 combine_kernel(BatchMeta meta, Shape sh, const float* __restrict__ part_o,
                const float2* __restrict__ part_ml, __nv_bfloat16* __restrict__ out) {
     constexpr int EPL = D / 32;
-    const CombineItem it = meta.combine[blockIdx.x];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int gw = blockIdx.x * 4 + (threadIdx.x >> 5);
+    int lo = 0, hi = meta.n_combine - 1;                  // last item with row_base <= w
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (meta.combine[mid].row_base <= gw) lo = mid; else hi = mid - 1;
+    }
+    const CombineItem it = meta.combine[lo];
     const int R = it.q_tokens * sh.G;
-    const int r = blockIdx.y * 4 + warp;
-    if (r >= R) return;
+    const int r = gw - it.row_base;
+    if (r >= R) return;                                   // past the last row
     const int64_t base = (int64_t)it.partial_row + r;
     float M = -INFINITY;
     for (int s0 = 0; s0 < it.n_splits; s0 += 32) {

@@ -178,8 +178,16 @@ def config_b2048_prefill(seed: int = 0) -> BatchSpec:
     return _subset(config_b2048(seed), lambda q: q > 1, "b2048pf")
 
 
+def config_small_decode(seed: int = 0) -> BatchSpec:
+    """A decode-only round as the trace run sees most of the time: 12 long-context decodes
+    (context uniform in [8192, 32768]), 8B shape.  Load balance needs the key ranges split."""
+    rng = np.random.default_rng(seed)
+    ctx = rng.integers(8192, 32769, size=12)
+    return make_spec("dec12", 32, 8, 128, 16, 65536, [1] * 12, list(ctx - 1), seed, rng)
+
+
 CONFIGS = {"tiny": config_tiny, "b512": config_b512, "b2048": config_b2048,
-           "70b": config_70b, "b2048dec": config_b2048_decodes, "b2048pf": config_b2048_prefill}
+           "70b": config_70b, "b2048dec": config_b2048_decodes, "b2048pf": config_b2048_prefill, "dec12": config_small_decode}
 
 
 def random_spec(seed: int, Hq=8, Hkv=2, D=64, B=16, n_prefill=3, n_decode=5,
