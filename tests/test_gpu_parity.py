@@ -191,3 +191,55 @@ def test_stress_long_decodes_with_chunk_no_deadlock():
     got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)[tok, head]
     gu.assert_close(got, want, "stress")
     ctx.close()
+
+
+@pytest.mark.parametrize("seed", range(100, 112))
+def test_fuzz_shapes_against_oracle(seed):
+    """Randomised shapes: every supported group size, both head dims, ragged chunks, contexts long enough
+    for split key ranges and several tiles per item, decodes and chunks in random order."""
+    rng = np.random.default_rng(seed)
+    G = int(rng.choice([1, 2, 4, 8, 16]))
+    Hkv = int(rng.choice([1, 2, 4]))
+    D = int(rng.choice([64, 128]))
+    spec = wl.random_spec(seed, Hq=G * Hkv, Hkv=Hkv, D=D, n_prefill=int(rng.integers(0, 5)), n_decode=int(rng.integers(0, 24)),
+                          max_chunk=int(rng.choice([40, 300, 900])), max_ctx=int(rng.choice([100, 1500, 6000])))
+    if spec.T == 0:
+        pytest.skip("empty draw")
+    hv = wl.host_values(spec)
+    got, pool_after = gu.run_gpu_host_values(spec, hv, 0)
+    want, cache_after = gu.run_oracle_host_values(spec, hv)
+    gu.assert_close(got, want, spec.name)
+    assert np.array_equal(pool_after[spec.touched_pages()], cache_after)
+
+
+def test_repeated_launches_mixed_shapes_no_deadlock():
+    """Back-to-back launches over alternating batch shapes (tile-heavy, decode-heavy, mixed, split and
+    unsplit items): the persistent kernel's counters, rings and barrier phases must re-arm every time."""
+    import torch
+    dev = torch.device("cuda:0")
+    shapes = [([1] * 40 + [700, 333], list(range(500, 4500, 100)) + [2500, 0]),
+              ([1] * 3, [30000, 12, 7000]),
+              ([129, 1, 64, 1, 1, 2047], [0, 999, 4096, 1, 127, 9000]),
+              ([1] * 200, [int(x) for x in np.random.default_rng(3).integers(1, 3000, 200)])]
+    runs = []
+    for k, (q_len, ctx_off) in enumerate(shapes):
+        spec = wl.make_spec(f"rep{k}", 32, 8, 128, 16, 24000, q_len, ctx_off, seed=k)
+        q, k_new, v_new, pool, compact = wl.device_values(spec, dev)
+        out = torch.empty((spec.T, spec.Hq, spec.D), device=dev, dtype=torch.bfloat16)
+        runs.append((spec, q, k_new, v_new, pool, compact, out))
+    ctx = binding.Context(32, 8, 128, 24000, 16, max_tokens=4096, max_reqs=256, max_total_pages=24000)
+    for it in range(300):
+        spec, q, k_new, v_new, pool, compact, out = runs[it % len(runs)]
+        ctx.cp_build_batch(spec.q_len, spec.ctx_off, spec.block_tables)
+        ctx.cp_attention_step(0, q, k_new if it < len(runs) else None, v_new if it < len(runs) else None, pool, out)
+    torch.cuda.synchronize()
+    ctx.cp_latency_table()
+    for spec, q, k_new, v_new, pool, compact, out in runs:
+        cache = gu.to_bits(compact)
+        tabs = spec.compact_tables()
+        ora.kv_append(gu.to_bits(k_new), gu.to_bits(v_new), cache, spec.q_len, spec.ctx_off, tabs)
+        tok, head = gu.sample_rows(spec, 64)
+        want = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale, rows=(tok, head))
+        got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)[tok, head]
+        gu.assert_close(got, want, spec.name)
+    ctx.close()
