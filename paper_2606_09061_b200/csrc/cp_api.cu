@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <utility>
 #include <vector>
 
 #include "cp_internal.h"
@@ -29,6 +30,24 @@ using namespace cp;
     } while (0)
 
 namespace {
+
+// Launch with programmatic dependent launch: the kernel may become resident while its predecessor in
+// the stream is still running; it calls griddepcontrol.wait before it touches anything the
+// predecessor wrote, so only its prologue (and the launch latency) overlaps.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr{};
+    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
 
 constexpr int kRing = 4096;           // timed steps kept for cp_latency_table
 
@@ -489,7 +508,7 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
         const int grid = std::min(c->n_sm, m.n_work);
         if (c->use_dl) {
             dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
-            dl::attn_dl_kernel<D><<<grid, dl::kThreads, dl::Layout<D>::kTotal, stream>>>(p, *tmap);
+            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D>, dim3(grid), dim3(dl::kThreads), dl::Layout<D>::kTotal, stream, p, *tmap));
         } else {
             TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
             attn_tc_kernel<D><<<grid, kTcThreads, TcLayout<D>::kTotal, stream>>>(p, *tmap);
@@ -499,8 +518,8 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
         c->info.grid_attn = grid;
     }
     if (m.n_combine > 0) {
-        combine_kernel<D><<<(c->combine_rows + 3) / 4, 128, 0, stream>>>(m, c->shape, c->d_part_o, c->d_part_ml, out);
-        CP_CUDA(cudaGetLastError());
+        CP_CUDA(launch_pdl(combine_kernel<D>, dim3((c->combine_rows + 3) / 4), dim3(128), 0, stream, m, c->shape,
+                           (const float*)c->d_part_o, (const float2*)c->d_part_ml, out));
         ++*launches;
     }
     c->info.grid_combine = m.n_combine;

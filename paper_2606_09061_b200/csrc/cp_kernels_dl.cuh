@@ -845,6 +845,9 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
+    // up to here nothing written by the preceding kernels (KV append; the previous step) was read
+    ptx::grid_dep_wait();
+    ptx::grid_dep_launch();                              // the combine kernel may stage its launch
 
     // launch allocation: 128 registers per thread.  The two producer / MMA warpgroups give most of
     // their share to the tile softmax (a 128-column score row in registers) and the decode softmax.

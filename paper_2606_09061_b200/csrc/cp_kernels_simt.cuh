@@ -22,6 +22,7 @@ __device__ __forceinline__ int64_t slab_elem_offset(int64_t page, int kv, int he
 // ---------------------------------------------------------------------------------
 __global__ void kv_append_kernel(BatchMeta meta, Shape sh, const uint4* __restrict__ k_new,
                                  const uint4* __restrict__ v_new, __nv_bfloat16* __restrict__ cache) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the attention kernel may start its prologue
     const int chunks = sh.D / 8;                          // 16-byte chunks per row
     const int64_t total = (int64_t)meta.n_tokens * sh.Hkv * chunks * 2;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
@@ -136,6 +137,7 @@ __global__ void __launch_bounds__(128)
 combine_kernel(BatchMeta meta, Shape sh, const float* __restrict__ part_o,
                const float2* __restrict__ part_ml, __nv_bfloat16* __restrict__ out) {
     constexpr int EPL = D / 32;
+    asm volatile("griddepcontrol.wait;" ::: "memory");                  // the attention kernel's partials are visible
     const int lane = threadIdx.x & 31;
     const int gw = blockIdx.x * 4 + (threadIdx.x >> 5);
     int lo = 0, hi = meta.n_combine - 1;                  // last item with row_base <= w
