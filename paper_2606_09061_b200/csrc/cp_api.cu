@@ -162,7 +162,7 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     chk(cudaMalloc(&c->d_part_o, sizeof(float) * (size_t)c->max_partial_rows * D));
     chk(cudaMalloc(&c->d_part_ml, sizeof(float2) * (size_t)c->max_partial_rows));
     chk(cudaMalloc(&c->d_counter, sizeof(int32_t) * 4));
-#if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
+#if defined(CP_TC_PROF) || defined(CP_TC_PROF2) || defined(CP_TL)
     chk(cudaMalloc(&c->d_prof, sizeof(unsigned long long) * 32 * 1024));
     chk(cudaMemset(c->d_prof, 0, sizeof(unsigned long long) * 32 * 1024));
 #endif
@@ -620,7 +620,7 @@ extern "C" int cp_set_memory_stats(cp_ctx* c, float used, float freemb, float al
     return CP_OK;
 }
 
-#if defined(CP_TC_PROF) || defined(CP_TC_PROF2)
+#if defined(CP_TC_PROF) || defined(CP_TC_PROF2) || defined(CP_TL)
 // debug builds only (not part of include/cp.h): per-CTA wait-time profile of the last launch
 extern "C" int cp_debug_prof(cp_ctx* c, unsigned long long* host_buf, int n_ctas) {
     if (!c->d_prof) return CP_ESTATE;

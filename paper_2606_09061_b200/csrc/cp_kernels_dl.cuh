@@ -50,6 +50,12 @@ constexpr int kTmemCols = 512;
 __host__ __device__ constexpr uint32_t col_s(int lane, uint32_t buf) { return lane == 0 ? buf * 128u : 448u + buf * 16u; }
 __host__ __device__ constexpr uint32_t col_o(int lane) { return lane == 0 ? 256u : 480u; }
 constexpr uint32_t kColQ = 384;
+#ifndef DL_POLY_EVERY
+#define DL_POLY_EVERY 0
+#endif
+// tile kind: every kPolyEvery-th exponential runs on the FMA pipe (0 = none).  Measured on B200: 4 -> -3.5 % on
+// chunk-only batches, +3 % on the mixed batch (the extra FMA-pipe instructions compete with the decode lane): off.
+constexpr int kPolyEvery = DL_POLY_EVERY;
 constexpr float kRescaleThreshold = 8.0f;      // log2 units: rescale O only when the max grew > 2^8
 constexpr uint32_t kSmallBytes = 12288;        // per lane: Q^T (4 KiB) + double-buffered P^T (8 KiB)
 
@@ -75,6 +81,15 @@ struct Layout {
 #else
 #define DL_T0 do {} while (0)
 #define DL_ACC(id) do {} while (0)
+#endif
+
+// Optional event timeline of CTA 0, lane T (build with -DCP_TL; debugging aid only): records
+// (event id, half-tile counter, clock) triples into p.prof.
+#ifdef CP_TL
+// cheap recording: 32-bit clock into the (idle) lane-S K/V ring of CTA 0, slot [half-tile][event]; copied out at the end
+#define DL_TL(ev, idx) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (idx) < 1024u) { unsigned c__; asm volatile("mov.u32 %0, %%clock;" : "=r"(c__)); reinterpret_cast<volatile unsigned*>(reinterpret_cast<uint8_t*>(ls) - Layout<D>::kOffMisc + kStagesT * Layout<D>::kSlotBytes)[(idx) * 16 + (ev)] = c__; } } while (0)
+#else
+#define DL_TL(ev, idx) do {} while (0)
 #endif
 
 struct LaneState {              // one per lane, in the misc region
@@ -118,6 +133,11 @@ struct Params {
     int32_t* counters;          // [0] next tile item, [1] next swap item, [2] finished CTAs
     unsigned long long* prof;   // [grid][16] role wait-time profile (-DCP_TC_PROF builds), else unused
 };
+
+// element e of a half-tile row: MUFU or FMA-pipe exponential (e is a constant after unrolling)
+__device__ __forceinline__ float ex2_sel(float x, int e) {
+    return (kPolyEvery > 0 && e % (kPolyEvery > 0 ? kPolyEvery : 1) == (kPolyEvery > 0 ? kPolyEvery : 1) - 1) ? ptx::ex2_poly(x) : ptx::ex2(x);
+}
 
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
     __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
@@ -290,7 +310,9 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
             const uint32_t slot = ld % kStages;
             DL_T0;
             if (j >= 4) ptx::mbar_wait(&ls->pv_issued[buf], ((g - 4) >> 2) & 1);      // PV(j-4) (same S buffer) is in the pipe
+            DL_TL(1, g);
             if (h == 0) ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+            DL_TL(2, g);
             DL_ACC(4);
             ptx::tc_fence_after();
             const uint32_t k_half = kv_base + slot * L::kSlotBytes + h * 8 * L::kGroupBytes;   // rows 64 h .. 64 h + 63
@@ -305,14 +327,17 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
                 ptx::umma_commit(&ls->ts_full[buf]);
             }
             __syncwarp();
+            DL_TL(3, g);
             DL_ACC(11);
         } else {
             const uint32_t ld = ld_base + (t == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * t + 2);
             const uint32_t slot = ld % kStages;
             DL_T0;
             ptx::mbar_wait(&ls->tp_full[buf], (g >> 2) & 1);
+            DL_TL(4, g);
             DL_ACC(5);
             if (h == 0) ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+            DL_TL(5, g);
             DL_ACC(6);
             ptx::tc_fence_after();
             const uint32_t v_half = kv_base + slot * L::kSlotBytes + h * 4 * L::kPageBytes;     // keys 64 h .. 64 h + 63
@@ -329,6 +354,7 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
                 ptx::mbar_arrive(&ls->pv_issued[buf]);
             }
             __syncwarp();
+            DL_TL(6, g);
             DL_ACC(12);
         }
     }
@@ -521,6 +547,7 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         const uint32_t buf = gh & 3;
         const uint32_t t_s = t_row + buf * 64;
         ptx::mbar_wait(&ls->ts_full[buf], (gh >> 2) & 1);
+        if (lane_base == 0) DL_TL(7, gh);
         DL_ACC(0);
         ptx::tc_fence_after();
 #ifdef DL_X_NOTMEM
@@ -530,6 +557,7 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         ptx::tmem_ld32(t_s, sr);
         ptx::tmem_ld32(t_s + 32, sr + 32);
         ptx::tmem_wait_ld();
+        if (lane_base == 0) DL_TL(8, gh);
 #ifdef DL_X_NOSOFTMAX
         { uint32_t pk[32];
 #pragma unroll
@@ -555,26 +583,29 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
             rescale = true;
         }
         const float neg_m = (m_ref == -INFINITY) ? 0.f : -m_ref;
+        if (lane_base == 0) DL_TL(9, gh);
         float sm[4] = {0.f, 0.f, 0.f, 0.f};             // independent sum chains
         uint32_t pk[32];                                // 64 scores -> 32 packed P columns
         if (nvalid == 64) {
 #pragma unroll
             for (int i = 0; i < 64; i += 2) {
-                const float a = ptx::ex2(fmaf(__uint_as_float(sr[i]), scale, neg_m));
-                const float b = ptx::ex2(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m));
+                const float a = ex2_sel(fmaf(__uint_as_float(sr[i]), scale, neg_m), i);
+                const float b = ex2_sel(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1);
                 sm[(i >> 1) & 3] += a + b;
                 pk[i >> 1] = pack_bf16(a, b);
             }
         } else {
 #pragma unroll
             for (int i = 0; i < 64; i += 2) {
-                const float a = i < nvalid ? ptx::ex2(fmaf(__uint_as_float(sr[i]), scale, neg_m)) : 0.f;
-                const float b = i + 1 < nvalid ? ptx::ex2(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m)) : 0.f;
+                const float a = i < nvalid ? ex2_sel(fmaf(__uint_as_float(sr[i]), scale, neg_m), i) : 0.f;
+                const float b = i + 1 < nvalid ? ex2_sel(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1) : 0.f;
                 sm[(i >> 1) & 3] += a + b;
                 pk[i >> 1] = pack_bf16(a, b);
             }
         }
+        if (lane_base == 0) DL_TL(10, gh);
         ptx::tmem_st32(t_s, pk);
+        if (lane_base == 0) DL_TL(11, gh);
         l = l * alpha + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
         if (j > 0 && __any_sync(0xffffffffu, rescale)) {
             ptx::mbar_wait(&ls->tpv_done[(gh - 1) & 3], ((gh - 1) >> 2) & 1);      // PV(j-1) (and all before) done: O readable
@@ -592,6 +623,7 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         ptx::tmem_wait_st();
         ptx::tc_fence_before();
         warp_arrive(&ls->tp_full[buf]);
+        if (lane_base == 0) DL_TL(12, gh);
         DL_ACC(1);
         ++gh;
     }
@@ -868,6 +900,9 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 6) ptx::tmem_dealloc(misc->tmem_base, kTmemCols);
+#ifdef CP_TL
+    if (blockIdx.x == 0 && p.prof) for (uint32_t i = threadIdx.x; i < 16384; i += kThreads) p.prof[i] = reinterpret_cast<const unsigned*>(smem + kStagesT * L::kSlotBytes)[i];
+#endif
 #ifdef CP_TC_PROF
     if (threadIdx.x == 0) { misc->lane[0].prof[15] = (unsigned long long)(clock64() - t_start__); misc->lane[0].prof[13] -= (unsigned long long)t_start__; }
     __syncthreads();
