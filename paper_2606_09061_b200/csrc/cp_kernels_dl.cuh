@@ -86,8 +86,9 @@ struct Layout {
 // Optional event timeline of CTA 0, lane T (build with -DCP_TL; debugging aid only): records
 // (event id, half-tile counter, clock) triples into p.prof.
 #ifdef CP_TL
-// cheap recording: 32-bit clock into the (idle) lane-S K/V ring of CTA 0, slot [half-tile][event]; copied out at the end
-#define DL_TL(ev, idx) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (idx) < 1024u) { unsigned c__; asm volatile("mov.u32 %0, %%clock;" : "=r"(c__)); reinterpret_cast<volatile unsigned*>(reinterpret_cast<uint8_t*>(ls) - Layout<D>::kOffMisc + kStagesT * Layout<D>::kSlotBytes)[(idx) * 16 + (ev)] = c__; } } while (0)
+// cheap recording: 32-bit clock into lane T's small region (idle during tile items) of CTA 0, slot [half-tile][event];
+// copied out at the end.  190 half-tiles fit.
+#define DL_TL(ev, idx) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (idx) < 190u) { unsigned c__; asm volatile("mov.u32 %0, %%clock;" : "=r"(c__)); reinterpret_cast<volatile unsigned*>(reinterpret_cast<uint8_t*>(ls) - Layout<D>::kOffMisc + (kStagesT + kStagesS) * Layout<D>::kSlotBytes)[(idx) * 16 + (ev)] = c__; } } while (0)
 #else
 #define DL_TL(ev, idx) do {} while (0)
 #endif
@@ -243,10 +244,16 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             const uint32_t slot = ld % kStages;
             { DL_T0; ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1); DL_ACC(8); }
             const bool leader = ptx::elect_one();
-#ifdef DL_X_NOTMA
-            if (leader) ptx::mbar_arrive(&ls->kv_full[slot]);
+#if defined(DL_X_NOTMA) || defined(DL_X_S_NOTMA)
+#ifdef DL_X_S_NOTMA
+            const bool no_tma = LANE == 1;
+#else
+            const bool no_tma = true;
+#endif
+            if (leader) { if (no_tma) ptx::mbar_arrive(&ls->kv_full[slot]); else ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u); }
             uint8_t* dst = kv_base + slot * L::kSlotBytes;
-            for (int j = 0; j < 0; ++j) {
+#pragma unroll
+            for (int j = 0; j < (no_tma ? 0 : 8); ++j) {
 #else
             if (leader) ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u);
             uint8_t* dst = kv_base + slot * L::kSlotBytes;
@@ -901,7 +908,7 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     __syncthreads();
     if (warp == 6) ptx::tmem_dealloc(misc->tmem_base, kTmemCols);
 #ifdef CP_TL
-    if (blockIdx.x == 0 && p.prof) for (uint32_t i = threadIdx.x; i < 16384; i += kThreads) p.prof[i] = reinterpret_cast<const unsigned*>(smem + kStagesT * L::kSlotBytes)[i];
+    if (blockIdx.x == 0 && p.prof) for (uint32_t i = threadIdx.x; i < 190 * 16; i += kThreads) p.prof[i] = reinterpret_cast<const unsigned*>(smem + (kStagesT + kStagesS) * L::kSlotBytes)[i];
 #endif
 #ifdef CP_TC_PROF
     if (threadIdx.x == 0) { misc->lane[0].prof[15] = (unsigned long long)(clock64() - t_start__); misc->lane[0].prof[13] -= (unsigned long long)t_start__; }
