@@ -48,11 +48,17 @@ def percentile(x, p):
 def run_trace(trace, *, Hq=32, Hkv=8, D=128, B=16, layers=32, pages_per_layer=20480,
               sched_kw: Optional[dict] = None, seed=0, device=0, kernel_variant=0,
               hook: Optional[Callable] = None, max_iters: Optional[int] = None,
-              overhead_us: int = 0):
+              overhead_us: int = 0, layer_gemms: bool = False, d_model: int = 4096, d_ff: int = 14336):
     """Run the whole trace.  `hook(it, batch, layer_tensors)` (tests only) is called after an
     iteration's steps were issued and synchronised, with batch = [(req_id, q_len, ctx_off,
     pages)] and layer_tensors(l) -> (q, k_new, v_new, pool_l, out_l).  Returns a report dict
-    plus the per-iteration measured microseconds (what the scheduler was told)."""
+    plus the per-iteration measured microseconds (what the scheduler was told).
+
+    layer_gemms=True adds, per layer, the dense projections of a Llama-shaped
+    block around the attention step -- QKV, O, gate/up, down as plain library GEMMs (torch.matmul =
+    cuBLAS) on seeded random bf16 weights shared by all layers -- so that the iteration time the
+    scheduler sees is that of a whole forward pass; it is timed with CUDA events around the whole
+    iteration.  The GEMMs are filler for the clock, not part of libcp."""
     import torch
     dev = torch.device(f"cuda:{device}")
     torch.cuda.set_device(dev)
@@ -80,6 +86,20 @@ def run_trace(trace, *, Hq=32, Hkv=8, D=128, B=16, layers=32, pages_per_layer=20
     ctx.cp_set_memory_stats((total_b - free_b) / 2**20, free_b / 2**20,
                             torch.cuda.memory_allocated(dev) / 2**20, torch.cuda.memory_reserved(dev) / 2**20)
 
+    if layer_gemms:
+        gw = lambda k, n: (torch.randn((k, n), generator=g, device=dev, dtype=torch.float32) * 0.02).bfloat16()
+        w_qkv, w_o = gw(d_model, (Hq + 2 * Hkv) * D), gw(Hq * D, d_model)
+        w_gu, w_dn = gw(d_model, 2 * d_ff), gw(d_ff, d_model)
+        x_buf = torch.randn((B_max, d_model), generator=g, device=dev, dtype=torch.float32).bfloat16()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def dense_part(T):
+        x = x_buf[:T]
+        qkv = x @ w_qkv                                        # the attention inputs stay the seeded banks
+        h = (x @ w_gu)
+        y = (torch.nn.functional.silu(h[:, :d_ff]) * h[:, d_ff:]) @ w_dn
+        return qkv, y, out[0, :T].reshape(T, Hq * D) @ w_o
+
     digest = hashlib.sha256()
     now, n_it, tokens = 0, 0, 0
     iter_us_log, classes = [], {"decode_only": [], "mixed": [], "prefill_only": []}
@@ -92,10 +112,20 @@ def run_trace(trace, *, Hq=32, Hkv=8, D=128, B=16, layers=32, pages_per_layer=20
             now = sched.cp_sched_next_arrival()
             continue
         ctx.cp_build_batch(descs=sched.descs, n=n)
+        if layer_gemms:
+            T_it = sum(sched.descs[i].q_len for i in range(n))
+            ev0.record()
         for l in range(layers):
             ctx.cp_attention_step(l, q_p[l], k_p[l], v_p[l], pool_p[l], out_p[l])
+            if layer_gemms:
+                dense_part(T_it)
+        if layer_gemms:
+            ev1.record()
         rows = ctx.cp_latency_table(cap=layers)            # waits for the iteration (H6)
         us = float(sum(r.us for r in rows))
+        if layer_gemms:
+            ev1.synchronize()
+            us = ev0.elapsed_time(ev1) * 1e3                   # whole forward pass: attention + dense GEMMs
         iter_us = max(1, int(round(us)) + overhead_us)
         r0 = rows[0]
         cls = "decode_only" if r0.n_prefill == 0 else ("prefill_only" if r0.n_decode == 0 else "mixed")
@@ -152,12 +182,14 @@ def main():
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--max-iters", type=int, default=None)
     ap.add_argument("--iter-us-out", default=None, help="write the measured iteration us (one per line)")
+    ap.add_argument("--layer-gemms", action="store_true", help="add the dense projections of each layer (library GEMMs) to the iteration time")
     a = ap.parse_args()
     from . import build
     build.build()
     trace = wl.make_trace(a.requests, rate_per_s=a.rate, seed=a.seed)
     report, log = run_trace(trace, layers=a.layers, pages_per_layer=a.pages_per_layer, seed=a.seed,
-                            sched_kw=dict(alpha=a.alpha, beta=a.beta, B_max=a.budget), max_iters=a.max_iters)
+                            sched_kw=dict(alpha=a.alpha, beta=a.beta, B_max=a.budget), max_iters=a.max_iters,
+                            layer_gemms=a.layer_gemms)
     report["arrival_rate_per_s"] = a.rate
     if a.iter_us_out:
         with open(a.iter_us_out, "w") as f:

@@ -167,3 +167,20 @@ def test_apc_ablation_shape_trace_on_gpu():
     kw_ref = dict(kw, page_mb=2 * Hkv * B * D * 2 * layers / 2**20)
     digest, n = replay_reference(trace, log, **kw_ref)
     assert n == len(log) and digest == report["schedule_sha256"]
+
+
+def test_reduced_trace_with_layer_gemms():
+    """the same loop with the dense projections of every layer (library GEMMs on seeded random
+    weights) inside the timed iteration; the schedule must still equal the reference replay on the measured times,
+    and iterations must take longer than the attention steps alone."""
+    build.build()
+    Hq, Hkv, D, B, layers = 32, 8, 128, 16, 2
+    trace = wl.make_trace(40, rate_per_s=2000.0, seed=4, short_median=200, long_lo=1500, long_hi=4000, out_median=16, out_max=48)
+    kw = dict(alpha=100.0, beta=-1.0, B_max=512, S_max=128, num_blocks=4096, block_size=B)
+    rep0, log0 = trace_run.run_trace(trace, Hq=Hq, Hkv=Hkv, D=D, B=B, layers=layers, pages_per_layer=4096, sched_kw=kw, seed=4)
+    rep1, log1 = trace_run.run_trace(trace, Hq=Hq, Hkv=Hkv, D=D, B=B, layers=layers, pages_per_layer=4096, sched_kw=kw, seed=4,
+                                     layer_gemms=True)
+    assert rep1["e2e_s"]["finished"] == 40
+    assert np.mean(log1) > np.mean(log0)
+    digest, n = replay_reference(trace, log1, **dict(kw, page_mb=2 * Hkv * B * D * 2 * layers / 2**20))
+    assert n == len(log1) and digest == rep1["schedule_sha256"]
