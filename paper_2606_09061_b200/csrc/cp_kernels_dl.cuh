@@ -8,7 +8,7 @@
 //   lane T  chunk tiles (kKindTile); when the tile list is exhausted it also pulls decode items
 //   lane S  decode / <=16-row items (kKindSwap) only
 //
-// Each lane owns a TMA producer warp, an MMA issuer warp, four softmax warps, a K/V tile ring in
+// Each lane owns its TMA producer warps, MMA issuer warp(s), four softmax warps, a K/V tile ring in
 // shared memory, its TMEM columns and its mbarriers; the lanes share nothing but the SM.
 //
 //   warpgroups 0-1: warps 0-2 TMA producers T, warps 3-4 TMA producers S, warps 5-6 MMA T (score
@@ -16,11 +16,12 @@
 //   warpgroup 2:    softmax T (thread <-> Q-tile row; also the decode items lane T runs once the
 //                   tile list is exhausted: thread <-> key)                         (232 regs)
 //   warpgroup 3:    softmax S (thread <-> key of the tile)                         (160 regs)
-// (Measured alternatives, round 1: splitting a score tile over two softmax warpgroups, and
-// reading the score row in chunks, were no faster -- see DESIGN.md section 6.)
+// (Measured alternatives, round 1 -- two softmax warpgroups per score tile or taking half-tiles in
+// turn, chunked score reads, software-pipelined score loads, L2 prefetch, other ring splits -- are
+// in DESIGN.md section 7 with their timelines.)
 //
-//   kKindTile   S[128 rows x 64 keys] = Q K^T per half-tile, with Q held in TMEM (A operand from TMEM, written
-//               once per item with tcgen05.st), P written back over S in TMEM as bf16 and consumed
+//   kKindTile   S[128 rows x 64 keys] = Q K^T per half-tile (four S buffers in flight), with Q held
+//               in TMEM (A operand from TMEM, written once per item with tcgen05.st), P written back over S in TMEM as bf16 and consumed
 //               as the A operand of O[128 x D] += P V.  Neither Q nor P touches shared memory, so
 //               the smem crossbar carries only the K/V tiles (TMA writes + one MMA read each).
 //   kKindSwap   <= 16 rows, D = 128: S^T[128 keys x 16] = K Q^T, O^T[128 d x 16] += V^T P^T.
