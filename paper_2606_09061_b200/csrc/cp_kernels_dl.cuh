@@ -22,8 +22,9 @@
 //
 //   kKindTile   S[128 rows x 64 keys] = Q K^T per half-tile (four S buffers in flight), with Q held
 //               in TMEM (A operand from TMEM, written once per item with tcgen05.st), P written back
-//               over S in TMEM as bf16 and consumed as the A operand of O[128 x D] += P V.  Neither Q nor P touches shared memory, so
-//               the smem crossbar carries only the K/V tiles (TMA writes + one MMA read each).
+//               over S in TMEM as bf16 and consumed as the A operand of O[128 x D] += P V.  Neither Q
+//               nor P touches shared memory, so the smem crossbar carries only the K/V tiles (TMA
+//               writes + one MMA read each).
 //   kKindSwap   <= 16 rows, D = 128: S^T[128 keys x 16] = K Q^T, O^T[128 d x 16] += V^T P^T.
 //
 // Operation: include/cp.h / DESIGN.md section 2.  Masking is by select, masked P is exactly 0.
