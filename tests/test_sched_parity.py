@@ -140,3 +140,21 @@ def test_config5_trace_bit_exact():
     _, n_it = run_both(tr, alpha=100.0, beta=-1.0, B_max=2048, S_max=1024, num_blocks=20480,
                        max_iters=2_000_000)
     assert n_it > 10000
+
+
+def test_trace_run_record_packing_matches_reference_packing():
+    """trace_run hashes the C descriptors directly (pack_batch); the reference replay hashes
+    pack_record of Python tuples: the two encodings must be byte-identical."""
+    from paper_2606_09061_b200 import trace_run
+    kw = dict(alpha=100.0, beta=-1.0, B_max=64, S_max=8, num_blocks=256)
+    cpp = binding.Scheduler(**{**kw, "max_batch": 8})
+    for rid, (a, p, o) in enumerate([(0, 70, 3), (5, 9, 2), (9, 130, 4)]):
+        cpp.cp_sched_add_request(rid, a, p, o)
+    t = 0
+    for _ in range(6):
+        n = cpp.cp_sched_next(t)
+        assert trace_run.pack_batch(cpp.descs, n) == rs.pack_record(cpp.batch())
+        if n == 0:
+            break
+        cpp.cp_sched_commit(50)
+        t += 50
