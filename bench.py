@@ -207,6 +207,16 @@ def run_ours(args):
     rows = ctx.cp_latency_table()
     step_us = np.array([r.us for r in rows], dtype=np.float64)
     info = ctx.cp_get_batch_info()
+    # H1 on its own ("cp_build_batch timed and reported separately"): host time of the call
+    # (validate + plan + pack + enqueue one H2D), median of 20, queue drained between calls
+    bb = []
+    for _ in range(20):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.cp_build_batch(descs=descs, n=spec.n_reqs)
+        bb.append((time.perf_counter() - t0) * 1e6)
+    torch.cuda.synchronize()
+    build_batch_us = float(np.median(bb))
 
     # ---- e2e: same metric through the C ABI with HOST buffers ------------------------------
     # Every step copies its Q / new K / new V from pinned host memory and reads its output back.  The
@@ -294,7 +304,10 @@ def run_ours(args):
         "iteration_us": {"step_incl_build_batch": ms_per_step * 1e3, "attention_step_mean": attn_us,
                          "attention_step_median": float(np.median(step_us)) if len(step_us) else None,
                          "attention_step_min": float(step_us.min()) if len(step_us) else None,
-                         "host_issue_per_step": t_host_issue / args.steps * 1e6},
+                         "attention_step_p10": float(np.percentile(step_us, 10)) if len(step_us) else None,
+                         "attention_step_p90": float(np.percentile(step_us, 90)) if len(step_us) else None,
+                         "host_issue_per_step": t_host_issue / args.steps * 1e6,
+                         "build_batch_host_median": build_batch_us, "build_batch_h2d_bytes": int(meta_bytes)},
         "tflops": flops_alg / (attn_us * 1e-6) / 1e12, "gbs": bytes_alg / (attn_us * 1e-6) / 1e9,
         "roofline": {"bound": bound, "achieved": achieved, "peak": peak, "unit": runit,
                      "frac": achieved / peak, "traffic": ncu_traffic(spec.name) if args.variant == 0 else None, "peak_source": peaks["source"],
@@ -335,7 +348,7 @@ def run_reference(args):
         hv = wl.host_values(spec)
         qb, kb, vb, cache = hv.q, hv.k_new, hv.v_new, hv.cache
     ora.kv_append(kb, vb, cache, spec.q_len, spec.ctx_off, spec.compact_tables())
-    per_step_s = max(2.0, min(20.0, 120.0 / (args.steps + args.warmup)))
+    per_step_s = max(1.0, min(20.0, 120.0 / (args.steps + args.warmup)))
     vals, descs, threads = [], [], 1
     for i in range(args.warmup + args.steps):
         v, threads, desc = oracle_sample_rate(spec, qb, cache, per_step_s, seed=i)
@@ -354,8 +367,8 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="b2048", choices=sorted(wl.CONFIGS))
     ap.add_argument("--variant", type=int, default=0, help="cp_config.kernel_variant")
