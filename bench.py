@@ -177,9 +177,13 @@ def run_ours(args):
     ctx.cp_set_memory_stats((total_b - free_b) / 2**20, free_b / 2**20,
                             torch.cuda.memory_allocated(dev) / 2**20, torch.cuda.memory_reserved(dev) / 2**20)
 
+    if args.rope:                                          # rotary embedding fused into the append
+        ctx.cp_enable_rope(binding.rope_inv_freq(spec.D))
+    attention_step = ctx.cp_attention_step_rope if args.rope else ctx.cp_attention_step
+
     def step():
         ctx.cp_build_batch(descs=descs, n=spec.n_reqs)
-        ctx.cp_attention_step(0, q, k_new, v_new, pool, out)
+        attention_step(0, q, k_new, v_new, pool, out)
 
     def barrier():
         if world > 1:
@@ -242,7 +246,7 @@ def run_ours(args):
         s_cmp.wait_event(b["h2d"])
         s_cmp.wait_event(b["d2h"])                      # its previous output has been read back
         ctx.cp_build_batch(descs=descs, n=spec.n_reqs, stream=s_cmp.cuda_stream)
-        ctx.cp_attention_step(0, b["q"], b["k"], b["v"], pool, b["out"], stream=s_cmp.cuda_stream)
+        attention_step(0, b["q"], b["k"], b["v"], pool, b["out"], stream=s_cmp.cuda_stream)
         b["cmp"].record(s_cmp)
         s_d2h.wait_event(b["cmp"])
         with torch.cuda.stream(s_d2h):
@@ -295,12 +299,12 @@ def run_ours(args):
                    "prefill_chunks": int((spec.q_len > 1).sum()), "sum_kv_len": int(spec.kv_len.sum()),
                    "pages": n_pages, "pool_pages": spec.num_blocks, "Hq": spec.Hq, "Hkv": spec.Hkv,
                    "D": spec.D, "block": spec.B, "layers_per_step": 1, "l2": "inputs_exceed_l2 (KV >> 126 MB), no flush",
-                   "parallelism": "replicas" if world > 1 else "single", "kernel_variant": args.variant,
+                   "parallelism": "replicas" if world > 1 else "single", "kernel_variant": args.variant, "rope": bool(args.rope),
                    "work_items": info.n_work_items, "combine_items": info.n_combine_items},
         "clocks": clocks,
         "e2e": {"value": whole_job_rate(spec.T, args.steps, world, e2e_ms), "unit": UNIT,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps},
-        "gpu_launches": int(info.kernels_per_step * args.steps),
+        "gpu_launches": int((info.kernels_per_step + (1 if args.rope else 0)) * args.steps),   # + rope_table_kernel of cp_build_batch
         "iteration_us": {"step_incl_build_batch": ms_per_step * 1e3, "attention_step_mean": attn_us,
                          "attention_step_median": float(np.median(step_us)) if len(step_us) else None,
                          "attention_step_min": float(step_us.min()) if len(step_us) else None,
@@ -372,6 +376,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="b2048", choices=sorted(wl.CONFIGS))
     ap.add_argument("--variant", type=int, default=0, help="cp_config.kernel_variant")
+    ap.add_argument("--rope", action="store_true",
+                    help="time cp_attention_step_rope (rotary embedding of Q / new K fused into the append)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

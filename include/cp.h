@@ -126,6 +126,30 @@ int cp_build_batch(cp_ctx* ctx, const cp_req_desc* reqs, int32_t n_reqs,
 int cp_attention_step(cp_ctx* ctx, int32_t layer, const void* q, const void* k_new,
                       const void* v_new, void* kv_cache, void* out, void* cuda_stream);
 
+/* N2 of SURVEY.md 8(f): rotary position embedding fused into the append (H2).  PAPER.md is
+ * silent on positional encoding (the execution backend is untouched); the
+ * definition is the textbook rotary embedding in the rotate-half pairing (R11): a row
+ * x of D elements at absolute position p = ctx_off + i becomes, for f in [0, D/2),
+ *     x'[f]       = x[f] cos(p w_f) - x[f + D/2] sin(p w_f)
+ *     x'[f + D/2] = x[f + D/2] cos(p w_f) + x[f] sin(p w_f)
+ * Angles and their cos / sin are evaluated in fp64 and rounded to fp32; products and sums are
+ * fp32 without fused multiply-add; the result is rounded to nearest even bf16 (R12).
+ *
+ * cp_enable_rope: inv_freq HOST [D/2] finite doubles (w_f; the usual choice is theta^(-2f/D)),
+ * copied.  A set-up call: allocates the rotated-Q workspace [max_tokens, Hq, D] bf16 and the
+ * (cos, sin) table [max_tokens, D/2], synchronises the device; may be called again to change the
+ * frequencies.  Batches built afterwards carry their table (one small kernel per cp_build_batch).
+ * Errors: CP_EINVAL, CP_ECUDA.
+ *
+ * cp_attention_step_rope: as cp_attention_step, but q and k_new are UNROTATED: K rows are rotated
+ * on their way into the pages, Q rows into the library's workspace (q itself is not modified), V
+ * rows are copied, all in the one append kernel; everything then attends as in cp_attention_step.
+ * k_new / v_new must not be NULL.  Errors: CP_ESTATE (cp_enable_rope not called, or the current
+ * batch was built before it), CP_EINVAL, CP_ECUDA. */
+int cp_enable_rope(cp_ctx* ctx, const double* inv_freq);
+int cp_attention_step_rope(cp_ctx* ctx, int32_t layer, const void* q, const void* k_new,
+                           const void* v_new, void* kv_cache, void* out, void* cuda_stream);
+
 /* H6: drain the ring of timed steps, oldest first, into rows (HOST, capacity cap);
  * *n_out receives the count.  Waits for the newest recorded step to finish.  The memory
  * features are what cp_set_memory_stats last stored (zeros if never called). */

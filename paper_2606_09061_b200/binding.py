@@ -26,6 +26,7 @@ EXPORTS = [
     "cp_sched_destroy", "cp_sched_add_request", "cp_sched_next", "cp_sched_commit",
     "cp_sched_next_arrival", "cp_sched_has_work", "cp_sched_get_stats",
     "cp_sched_request_times", "cp_sched_predict", "cp_sched_select_chunk",
+    "cp_enable_rope", "cp_attention_step_rope",
 ]
 
 
@@ -101,6 +102,8 @@ def load(path: Optional[str] = None):
     lib.cp_destroy.argtypes = [C.c_void_p]
     lib.cp_build_batch.argtypes = [C.c_void_p, C.POINTER(cp_req_desc), C.c_int32, C.c_void_p]
     lib.cp_attention_step.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
+    lib.cp_attention_step_rope.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
+    lib.cp_enable_rope.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     lib.cp_latency_table.argtypes = [C.c_void_p, C.POINTER(cp_latency_row), C.c_int32,
                                      C.POINTER(C.c_int32)]
     lib.cp_set_memory_stats.argtypes = [C.c_void_p] + [C.c_float] * 4
@@ -147,6 +150,11 @@ def make_descs(q_len: Sequence[int], ctx_off: Sequence[int], block_tables: Seque
     return arr, keep
 
 
+def rope_inv_freq(head_dim: int, theta: float = 10000.0) -> np.ndarray:
+    """The usual rotary frequencies w_f = theta^(-2f/D), float64 [D/2] (argument of cp_enable_rope)."""
+    return np.float64(theta) ** (-np.arange(0, head_dim, 2, dtype=np.float64) / head_dim)
+
+
 def _ptr(t) -> Optional[int]:
     if t is None:
         return None
@@ -181,6 +189,16 @@ class Context:
     def cp_attention_step(self, layer, q, k_new, v_new, kv_cache, out, stream=None):
         _check(self.lib.cp_attention_step(self.handle, layer, _ptr(q), _ptr(k_new), _ptr(v_new),
                                           _ptr(kv_cache), _ptr(out), _ptr(stream)))
+
+    def cp_enable_rope(self, inv_freq):
+        f = np.ascontiguousarray(inv_freq, dtype=np.float64)
+        if f.shape != (self.cfg.head_dim // 2,):
+            raise ValueError(f"inv_freq must have head_dim/2 = {self.cfg.head_dim // 2} entries")
+        _check(self.lib.cp_enable_rope(self.handle, f.ctypes.data_as(C.POINTER(C.c_double))))
+
+    def cp_attention_step_rope(self, layer, q, k_new, v_new, kv_cache, out, stream=None):
+        _check(self.lib.cp_attention_step_rope(self.handle, layer, _ptr(q), _ptr(k_new), _ptr(v_new),
+                                               _ptr(kv_cache), _ptr(out), _ptr(stream)))
 
     def cp_latency_table(self, cap=4096) -> List[cp_latency_row]:
         rows = (cp_latency_row * cap)()

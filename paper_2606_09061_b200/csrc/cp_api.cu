@@ -78,6 +78,11 @@ struct cp_ctx {
     float2* d_part_ml = nullptr;
     int32_t* d_counter = nullptr;      // persistent-kernel work counter
     unsigned long long* d_prof = nullptr;   // CP_TC_PROF builds only
+    // rotary embedding fused into the append (cp_enable_rope); all null / -1 until enabled
+    double* d_inv_freq = nullptr;      // [D/2]
+    float2* d_rope_cs = nullptr;       // [max_tokens][D/2] (cos, sin) of the current batch's positions
+    __nv_bfloat16* d_q_rot = nullptr;  // [max_tokens][Hq][D] rotated Q of the running step
+    int64_t rope_table_iter = -1;      // iter the table was computed for
     // pinned staging, double buffered
     uint8_t* h_stage[2] = {nullptr, nullptr};
     cudaEvent_t stage_done[2] = {nullptr, nullptr};
@@ -199,6 +204,9 @@ extern "C" int cp_destroy(cp_ctx* c) {
     cudaFree(c->d_part_ml);
     cudaFree(c->d_counter);
     cudaFree(c->d_prof);
+    cudaFree(c->d_inv_freq);
+    cudaFree(c->d_rope_cs);
+    cudaFree(c->d_q_rot);
     for (int i = 0; i < 2; ++i) {
         if (c->h_stage[i]) cudaFreeHost(c->h_stage[i]);
         if (c->stage_done[i]) cudaEventDestroy(c->stage_done[i]);
@@ -430,6 +438,42 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     c->n_decode = n_decode;
     c->have_batch = true;
     ++c->iter;
+    if (c->d_rope_cs && T > 0) {       // positions changed: (cos, sin) table of this batch, same stream as the copy
+        const int half = sh.D / 2;
+        const int grid = (int)std::min<int64_t>((T * half + 255) / 256, (int64_t)c->n_sm * 8);
+        rope_table_kernel<<<grid, 256, 0, stream>>>(m, half, c->d_inv_freq, c->d_rope_cs);
+        CP_CUDA(cudaGetLastError());
+    }
+    c->rope_table_iter = c->d_rope_cs ? c->iter : -1;
+    return CP_OK;
+}
+
+// N2: rotary embedding.  Allocates its workspace here (a set-up call, like cp_create).
+extern "C" int cp_enable_rope(cp_ctx* c, const double* inv_freq) {
+    if (!c || !inv_freq) { cp_set_error("cp_enable_rope: null argument"); return CP_EINVAL; }
+    const Shape& sh = c->shape;
+    const int half = sh.D / 2;
+    for (int i = 0; i < half; ++i)
+        if (!(inv_freq[i] == inv_freq[i]) || inv_freq[i] - inv_freq[i] != 0.0) {
+            cp_set_error("cp_enable_rope: inv_freq[%d] is not finite", i);
+            return CP_EINVAL;
+        }
+    CP_CUDA(cudaSetDevice(c->cfg.device));
+    if (!c->d_inv_freq) {
+        double* f = nullptr; float2* cs = nullptr; __nv_bfloat16* qr = nullptr;
+        cudaError_t e = cudaMalloc(&f, sizeof(double) * half);
+        if (e == cudaSuccess) e = cudaMalloc(&cs, sizeof(float2) * (size_t)c->cfg.max_tokens * half);
+        if (e == cudaSuccess) e = cudaMalloc(&qr, sizeof(__nv_bfloat16) * (size_t)c->cfg.max_tokens * sh.Hq * sh.D);
+        if (e != cudaSuccess) {
+            cudaFree(f); cudaFree(cs); cudaFree(qr);
+            cp_set_error("cp_enable_rope: CUDA allocation failed: %s", cudaGetErrorString(e));
+            return CP_ECUDA;
+        }
+        c->d_inv_freq = f; c->d_rope_cs = cs; c->d_q_rot = qr;
+    }
+    CP_CUDA(cudaDeviceSynchronize());                       // no step may still be reading the old table
+    CP_CUDA(cudaMemcpy(c->d_inv_freq, inv_freq, sizeof(double) * half, cudaMemcpyHostToDevice));
+    c->rope_table_iter = -1;                                // the current batch (if any) has no table yet
     return CP_OK;
 }
 
@@ -533,10 +577,18 @@ static int launch_tc(cp_ctx* c, const __nv_bfloat16* q, __nv_bfloat16* kv_cache,
 }
 #endif
 
-extern "C" int cp_attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new,
-                                 const void* v_new, void* kv_cache, void* out, void* stream_) {
+static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new, const void* v_new,
+                          void* kv_cache, void* out, void* stream_, bool rope) {
     if (!c) return CP_EINVAL;
     if (!c->have_batch) { cp_set_error("cp_attention_step: no batch built"); return CP_ESTATE; }
+    if (rope) {
+        if (!c->d_rope_cs) { cp_set_error("cp_attention_step_rope: cp_enable_rope was not called"); return CP_ESTATE; }
+        if (c->rope_table_iter != c->iter) {
+            cp_set_error("cp_attention_step_rope: the batch was built before cp_enable_rope");
+            return CP_ESTATE;
+        }
+        if (!k_new) { cp_set_error("cp_attention_step_rope: k_new / v_new must not be NULL"); return CP_EINVAL; }
+    }
     if (!q || !kv_cache || !out || ((k_new == nullptr) != (v_new == nullptr)) || layer < 0) {
         cp_set_error("cp_attention_step: bad argument");
         return CP_EINVAL;
@@ -552,7 +604,19 @@ extern "C" int cp_attention_step(cp_ctx* c, int32_t layer, const void* q, const 
     CP_CUDA(cudaEventRecord(ts.start, stream));
     int launches = 0;
     if (m.n_tokens > 0) {
-        if (k_new) {
+        if (rope) {
+            const Shape& sh = c->shape;
+            const int64_t total = (int64_t)m.n_tokens * (sh.Hkv * (sh.D / 8) + (sh.Hkv + sh.Hq) * (sh.D / 16));
+            const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 8);
+            kv_append_rope_kernel<<<grid, 256, 0, stream>>>(m, sh, static_cast<const uint4*>(q),
+                                                            static_cast<const uint4*>(k_new),
+                                                            static_cast<const uint4*>(v_new), c->d_rope_cs,
+                                                            static_cast<__nv_bfloat16*>(kv_cache),
+                                                            reinterpret_cast<uint4*>(c->d_q_rot));
+            CP_CUDA(cudaGetLastError());
+            ++launches;
+            q = c->d_q_rot;
+        } else if (k_new) {
             const int64_t total = (int64_t)m.n_tokens * c->shape.Hkv * (c->shape.D / 8) * 2;
             const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 8);
             kv_append_kernel<<<grid, 256, 0, stream>>>(m, c->shape, static_cast<const uint4*>(k_new),
@@ -593,6 +657,16 @@ extern "C" int cp_attention_step(cp_ctx* c, int32_t layer, const void* q, const 
     ++c->ring_head;
     if (c->ring_head - c->ring_tail > kRing) c->ring_tail = c->ring_head - kRing;   // oldest rows overwritten
     return CP_OK;
+}
+
+extern "C" int cp_attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new,
+                                 const void* v_new, void* kv_cache, void* out, void* stream) {
+    return attention_step(c, layer, q, k_new, v_new, kv_cache, out, stream, false);
+}
+
+extern "C" int cp_attention_step_rope(cp_ctx* c, int32_t layer, const void* q, const void* k_new,
+                                      const void* v_new, void* kv_cache, void* out, void* stream) {
+    return attention_step(c, layer, q, k_new, v_new, kv_cache, out, stream, true);
 }
 
 // ------------------------------------------------------------------------------------

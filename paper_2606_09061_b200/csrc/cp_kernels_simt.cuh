@@ -44,6 +44,98 @@ __global__ void kv_append_kernel(BatchMeta meta, Shape sh, const uint4* __restri
 }
 
 // ---------------------------------------------------------------------------------
+// N2: rotary position embedding fused into H2.
+// rope_table_kernel runs once per cp_build_batch: cs[tok][i] = (cos, sin)(pos_tok * w_i), the angle
+// and its cosine / sine in fp64 (an fp32 angle is off by 1e-2 rad at position 1e5), rounded to fp32.
+// kv_append_rope_kernel then does, per layer, in one pass over the step's new rows: V rows copied to
+// their page slots, K rows rotated on their way into the pages, Q rows rotated into `q_rot` (the Q the
+// attention kernel reads).  Rotate-half pairing (include/cp.h); fp32 products and sums without fused
+// multiply-add, round-to-nearest-even to bf16 -- the same decision oracle/rope.py takes.
+// ---------------------------------------------------------------------------------
+__global__ void rope_table_kernel(BatchMeta meta, int half, const double* __restrict__ inv_freq,
+                                  float2* __restrict__ cs) {
+    const int64_t total = (int64_t)meta.n_tokens * half;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int tok = (int)(i / half), f = (int)(i % half);
+        const int req = meta.tok_req[tok];
+        const int pos = meta.ctx_off[req] + (tok - meta.cu_q[req]);
+        double s, c;
+        sincos((double)pos * inv_freq[f], &s, &c);
+        cs[i] = make_float2((float)c, (float)s);
+    }
+}
+
+__device__ __forceinline__ void rope_rotate8(const uint4& lo, const uint4& hi, const float2* __restrict__ cs,
+                                             uint4& out_lo, uint4& out_hi) {
+    const __nv_bfloat162* l2 = reinterpret_cast<const __nv_bfloat162*>(&lo);
+    const __nv_bfloat162* h2 = reinterpret_cast<const __nv_bfloat162*>(&hi);
+    __nv_bfloat162* ol = reinterpret_cast<__nv_bfloat162*>(&out_lo);
+    __nv_bfloat162* oh = reinterpret_cast<__nv_bfloat162*>(&out_hi);
+    const float4* cs4 = reinterpret_cast<const float4*>(cs);          // two (cos, sin) pairs per load
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float4 t = cs4[j];
+        const float2 a = __bfloat1622float2(l2[j]), b = __bfloat1622float2(h2[j]);
+        const float lx = __fsub_rn(__fmul_rn(a.x, t.x), __fmul_rn(b.x, t.y));
+        const float hx = __fadd_rn(__fmul_rn(b.x, t.x), __fmul_rn(a.x, t.y));
+        const float ly = __fsub_rn(__fmul_rn(a.y, t.z), __fmul_rn(b.y, t.w));
+        const float hy = __fadd_rn(__fmul_rn(b.y, t.z), __fmul_rn(a.y, t.w));
+        ol[j] = __floats2bfloat162_rn(lx, ly);
+        oh[j] = __floats2bfloat162_rn(hx, hy);
+    }
+}
+
+// One thread per unit: a 16-byte chunk of a V row (copy), or the 16-byte chunk c of the lower half of a
+// K / Q row together with chunk c of its upper half (rotate).
+__global__ void kv_append_rope_kernel(BatchMeta meta, Shape sh, const uint4* __restrict__ q,
+                                      const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
+                                      const float2* __restrict__ cs, __nv_bfloat16* __restrict__ cache,
+                                      uint4* __restrict__ q_rot) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the attention kernel may start its prologue
+    const int chunks = sh.D / 8, hc = sh.D / 16, half = sh.D / 2;
+    const int v_units = sh.Hkv * chunks;
+    const int per_tok = v_units + (sh.Hkv + sh.Hq) * hc;
+    const int64_t total = (int64_t)meta.n_tokens * per_tok;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int tok = (int)(i / per_tok);
+        int r = (int)(i % per_tok);
+        const int req = meta.tok_req[tok];
+        const int pos = meta.ctx_off[req] + (tok - meta.cu_q[req]);
+        const int64_t page = meta.block_table[meta.bt_off[req] + pos / sh.B];
+        if (r < v_units) {
+            const int g = r / chunks, c = r % chunks;
+            __nv_bfloat16* dst = cache + slab_elem_offset(page, 1, g, sh.Hkv, sh.B, sh.D) +
+                                 (int64_t)(pos % sh.B) * sh.D + c * 8;
+            *reinterpret_cast<uint4*>(dst) = v_new[((int64_t)tok * sh.Hkv + g) * chunks + c];
+            continue;
+        }
+        r -= v_units;
+        const int head = r / hc, c = r % hc;
+        const float2* cs_row = cs + (int64_t)tok * half + c * 8;
+        uint4 lo, hi, olo, ohi;
+        if (head < sh.Hkv) {
+            const uint4* src = k_new + ((int64_t)tok * sh.Hkv + head) * chunks;
+            lo = src[c];
+            hi = src[hc + c];
+            rope_rotate8(lo, hi, cs_row, olo, ohi);
+            uint4* dst = reinterpret_cast<uint4*>(cache + slab_elem_offset(page, 0, head, sh.Hkv, sh.B, sh.D) +
+                                                  (int64_t)(pos % sh.B) * sh.D);
+            dst[c] = olo;
+            dst[hc + c] = ohi;
+        } else {
+            const int64_t row = ((int64_t)tok * sh.Hq + (head - sh.Hkv)) * chunks;
+            lo = q[row + c];
+            hi = q[row + hc + c];
+            rope_rotate8(lo, hi, cs_row, olo, ohi);
+            q_rot[row + c] = olo;
+            q_rot[row + hc + c] = ohi;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------
 // Reference attention: CTA per work item, warp per row, lane owns D/32 dims.
 // Scores are kept in log2 units (q pre-scaled by sm_scale * log2 e).
 // ---------------------------------------------------------------------------------
