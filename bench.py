@@ -74,7 +74,7 @@ class ClockSampler:
         time.sleep(0.15)
         self.proc.terminate()
         self.t.join(timeout=2)
-        sm, mx, reasons = [], None, set()
+        sm, pw, mx, reasons = [], [], None, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for l in self.lines:
             f = [x.strip() for x in l.split(",")]
@@ -84,11 +84,21 @@ class ClockSampler:
                 sm.append(float(f[0])); mx = float(f[1])
             except ValueError:
                 continue
+            try:
+                pw.append(float(f[2]))
+            except ValueError:
+                pass
             for n, v in zip(names, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
+        # power.draw is a running average that lags the load by ~1 s: the last quarter of the samples is
+        # the steady state of a long run (--steps 4000), the start of a short one
+        tail = pw[-max(1, len(pw) // 4):]
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm),
+                "sm_mhz_last_quarter": float(np.median(sm[-max(1, len(sm) // 4):])) if sm else None,
+                "power_w_last_quarter": float(np.mean(tail)) if tail else None,
+                "power_w_max": float(max(pw)) if pw else None}
 
 
 def oracle_sample_rate(spec, q_bits, cache_bits, target_s, seed=0):
@@ -310,6 +320,7 @@ def run_ours(args):
                          "attention_step_min": float(step_us.min()) if len(step_us) else None,
                          "attention_step_p10": float(np.percentile(step_us, 10)) if len(step_us) else None,
                          "attention_step_p90": float(np.percentile(step_us, 90)) if len(step_us) else None,
+                         "attention_step_last_quarter": float(step_us[-max(1, len(step_us) // 4):].mean()) if len(step_us) else None,
                          "host_issue_per_step": t_host_issue / args.steps * 1e6,
                          "build_batch_host_median": build_batch_us, "build_batch_h2d_bytes": int(meta_bytes)},
         "tflops": flops_alg / (attn_us * 1e-6) / 1e12, "gbs": bytes_alg / (attn_us * 1e-6) / 1e9,
