@@ -48,7 +48,8 @@ def percentile(x, p):
 def run_trace(trace, *, Hq=32, Hkv=8, D=128, B=16, layers=32, pages_per_layer=20480,
               sched_kw: Optional[dict] = None, seed=0, device=0, kernel_variant=0,
               hook: Optional[Callable] = None, max_iters: Optional[int] = None,
-              overhead_us: int = 0, layer_gemms: bool = False, d_model: int = 4096, d_ff: int = 14336):
+              overhead_us: int = 0, layer_gemms: bool = False, d_model: int = 4096, d_ff: int = 14336,
+              rope_inv_freq=None):
     """Run the whole trace.  `hook(it, batch, layer_tensors)` (tests only) is called after an
     iteration's steps were issued and synchronised, with batch = [(req_id, q_len, ctx_off,
     pages)] and layer_tensors(l) -> (q, k_new, v_new, pool_l, out_l).  Returns a report dict
@@ -58,7 +59,10 @@ def run_trace(trace, *, Hq=32, Hkv=8, D=128, B=16, layers=32, pages_per_layer=20
     block around the attention step -- QKV, O, gate/up, down as plain library GEMMs (torch.matmul =
     cuBLAS) on seeded random bf16 weights shared by all layers -- so that the iteration time the
     scheduler sees is that of a whole forward pass; it is timed with CUDA events around the whole
-    iteration.  The GEMMs are filler for the clock, not part of libcp."""
+    iteration.  The GEMMs are filler for the clock, not part of libcp.
+
+    rope_inv_freq (float64 [D/2]): every step goes through cp_attention_step_rope, i.e. the
+    Q / new-K banks are taken as unrotated and rotated by absolute position inside the append."""
     import torch
     dev = torch.device(f"cuda:{device}")
     torch.cuda.set_device(dev)
@@ -82,6 +86,9 @@ def run_trace(trace, *, Hq=32, Hkv=8, D=128, B=16, layers=32, pages_per_layer=20
 
     ctx = binding.Context(Hq, Hkv, D, pages_per_layer, B, num_layers=layers, max_tokens=B_max, max_reqs=S_max,
                           max_total_pages=pages_per_layer, device=device, kernel_variant=kernel_variant)
+    if rope_inv_freq is not None:
+        ctx.cp_enable_rope(rope_inv_freq)
+    attention_step = ctx.cp_attention_step if rope_inv_freq is None else ctx.cp_attention_step_rope
     free_b, total_b = torch.cuda.mem_get_info(dev)
     ctx.cp_set_memory_stats((total_b - free_b) / 2**20, free_b / 2**20,
                             torch.cuda.memory_allocated(dev) / 2**20, torch.cuda.memory_reserved(dev) / 2**20)
@@ -116,7 +123,7 @@ def run_trace(trace, *, Hq=32, Hkv=8, D=128, B=16, layers=32, pages_per_layer=20
             T_it = sum(sched.descs[i].q_len for i in range(n))
             ev0.record()
         for l in range(layers):
-            ctx.cp_attention_step(l, q_p[l], k_p[l], v_p[l], pool_p[l], out_p[l])
+            attention_step(l, q_p[l], k_p[l], v_p[l], pool_p[l], out_p[l])
             if layer_gemms:
                 dense_part(T_it)
         if layer_gemms:

@@ -13,7 +13,8 @@ import pytest
 
 from oracle import attention as ora
 from oracle import ref_scheduler as rs
-from paper_2606_09061_b200 import build, trace_run, workloads as wl
+from oracle import rope as orope
+from paper_2606_09061_b200 import binding, build, trace_run, workloads as wl
 from tests import gpu_util as gu
 
 pytestmark = pytest.mark.gpu
@@ -39,7 +40,7 @@ def replay_reference(trace, iter_us_log, **kw):
     return h.hexdigest(), i
 
 
-def make_parity_hook(Hq, Hkv, D, B, layers, every, n_rows, stats, scale):
+def make_parity_hook(Hq, Hkv, D, B, layers, every, n_rows, stats, scale, inv_freq=None):
     def hook(it, batch, layer_tensors):
         if it % every:
             return
@@ -55,9 +56,17 @@ def make_parity_hook(Hq, Hkv, D, B, layers, every, n_rows, stats, scale):
             q, k_new, v_new, pool_l, out_l = layer_tensors(l)
             cache = gu.to_bits(pool_l[touched])                       # AFTER the step's append
             before = cache.copy()
-            ora.kv_append(gu.to_bits(k_new), gu.to_bits(v_new), cache, q_len, ctx_off, spec.compact_tables())
-            assert np.array_equal(cache, before), "H2: GPU append differs from the oracle's"
-            want = ora.attention(gu.to_bits(q), cache, q_len, ctx_off, spec.compact_tables(), scale, rows=(tok, head))
+            q_bits, k_bits = gu.to_bits(q), gu.to_bits(k_new)
+            if inv_freq is not None:                                  # the step rotated Q and the new K rows
+                pos = orope.token_positions(q_len, ctx_off)
+                q_bits, k_bits = orope.rope_bf16(q_bits, pos, inv_freq), orope.rope_bf16(k_bits, pos, inv_freq)
+            ora.kv_append(k_bits, gu.to_bits(v_new), cache, q_len, ctx_off, spec.compact_tables())
+            if inv_freq is None:
+                assert np.array_equal(cache, before), "H2: GPU append differs from the oracle's"
+            else:                                                     # DESIGN.md R12: fp64 cos / sin last place
+                dk = np.abs(cache.astype(np.int32) - before.astype(np.int32))
+                assert dk.max() <= 1 and (dk != 0).sum() <= 2 + 1e-5 * spec.T * Hkv * D
+            want = ora.attention(q_bits, cache, q_len, ctx_off, spec.compact_tables(), scale, rows=(tok, head))
             got = wl.bf16_bits_to_f64(gu.to_bits(out_l)).reshape(spec.T, Hq, D)[tok, head]
             mx, mean = gu.assert_close(got, want, f"iteration {it} layer {l}")
             stats.append((it, l, mx, mean))
@@ -78,6 +87,26 @@ def test_reduced_trace_parity_and_schedule_identity():
     assert report["e2e_s"]["finished"] == 80 and report["ttft_s"]["started"] == 80
     assert report["iterations"] == len(log) > 100 and len(stats) >= 20
     assert report["iteration_us_by_class"]["mixed"]["iterations"] > 0
+    kw_ref = dict(kw, page_mb=2 * Hkv * B * D * 2 * layers / 2**20)
+    digest, n = replay_reference(trace, log, **kw_ref)
+    assert n == len(log) and digest == report["schedule_sha256"]
+
+
+def test_reduced_trace_with_rope():
+    """The serving loop through cp_attention_step_rope: same schedule identity, parity against the
+    rotated oracle on sampled iterations (pages carry rotated K from step to step)."""
+    build.build()
+    Hq, Hkv, D, B, layers = 32, 8, 128, 16, 2
+    trace = wl.make_trace(40, rate_per_s=2000.0, seed=5, short_median=200, long_lo=1500, long_hi=6000,
+                          out_median=24, out_max=96)
+    kw = dict(alpha=100.0, beta=-1.0, B_max=512, S_max=128, num_blocks=6144, block_size=B)
+    stats = []
+    scale = float(np.float32(1.0) / np.sqrt(np.float32(D)))
+    w = binding.rope_inv_freq(D, 500000.0)
+    hook = make_parity_hook(Hq, Hkv, D, B, layers, 7, 256, stats, scale, inv_freq=w)
+    report, log = trace_run.run_trace(trace, Hq=Hq, Hkv=Hkv, D=D, B=B, layers=layers, pages_per_layer=6144,
+                                      sched_kw=kw, seed=5, hook=hook, rope_inv_freq=w)
+    assert report["e2e_s"]["finished"] == 40 and len(stats) >= 10
     kw_ref = dict(kw, page_mb=2 * Hkv * B * D * 2 * layers / 2**20)
     digest, n = replay_reference(trace, log, **kw_ref)
     assert n == len(log) and digest == report["schedule_sha256"]
