@@ -179,12 +179,21 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
 // boundaries.  Page ids are prefetched 32 at a time (one per lane of the warp, two windows; each
 // producer's tile sequence is monotone) so no dependent global load sits between two TMA issues.
 // ------------------------------------------------------------------------------------------
-template <int D, int LANE>
-__device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tmap, uint8_t* smem, LaneState* ls, int lane, int pw) {
+// ONE copy of this code serves both lanes (LANE is a warp-uniform runtime value): the kernel's hot
+// instruction footprint has to stay inside the 32 KB L1.5 instruction cache of the SM -- with one copy
+// per lane (and the other per-lane duplicates) it was 39 KB in a mixed batch and the tile softmax spent
+// 40-50 % of its issue slots waiting for instruction fetch (ncu: stall_no_inst; 4 % in a chunk-only batch).
+template <int D>
+__device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tmap, uint8_t* smem, Misc* misc, int lane, int warp) {
     using L = Layout<D>;
-    constexpr int kStages = LANE == 0 ? kStagesT : kStagesS;
-    constexpr int kProd = LANE == 0 ? kProdT : kProdS;
-    uint8_t* kv_base = smem + L::kOffKv[LANE];
+    static_assert(kStagesT == kStagesS, "the shared producer code assumes one ring depth");
+    constexpr int kStages = kStagesT;
+    const int LANE = warp < kProdT ? 0 : 1;
+    const int pw = LANE == 0 ? warp : warp - kProdT;
+    const int kProd = LANE == 0 ? kProdT : kProdS;
+    LaneState* ls = &misc->lane[LANE];
+    constexpr uint32_t kOff0 = L::kOffKv[0], kOff1 = L::kOffKv[1];
+    uint8_t* kv_base = smem + (LANE == 0 ? kOff0 : kOff1);
     uint32_t ld_base = 0, item_cnt = 0;          // ld_base: tile loads of all previous items
     bool tiles_left = LANE == 0;
     for (;;) {
@@ -517,13 +526,14 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
                                              uint32_t& gh, int row, uint32_t lane_base) {
     const Shape& sh = p.sh;
     const int G = sh.G;
+    const int gs = 31 - __clz(G);                        // G is a power of two (cp_create): shifts, not divisions
     const int R = it.q_tokens * G;
     const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
     const int tok0 = p.meta.cu_q[it.req] + it.q_start;
     const int ctx = p.meta.ctx_off[it.req];
     const bool valid_row = row < R;
-    const int tok = tok0 + row / G;
-    const int head = it.kv_head * G + row % G;
+    const int tok = tok0 + (row >> gs);
+    const int head = it.kv_head * G + (row & (G - 1));
     const float scale = sh.sm_scale * 1.4426950408889634f;
     const uint32_t t_row = tmem + (lane_base << 16);
 
@@ -547,7 +557,7 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
     }
     DL_ACC(9);
 
-    const int limit = valid_row ? min(it.kv_end, ctx + it.q_start + row / G + 1) : 0;   // causal, diagonal inclusive
+    const int limit = valid_row ? min(it.kv_end, ctx + it.q_start + (row >> gs) + 1) : 0;   // causal, diagonal inclusive
     float m_ref = -INFINITY, l = 0.f;
     const int nh = (it.kv_end - it.kv_begin + 63) / 64;          // 64-key half-tiles, S buffer = gh & 3
 
@@ -678,6 +688,8 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
     constexpr int D = 128;
     const Shape& sh = p.sh;
     const int G = sh.G;
+    const int gs = 31 - __clz(G);                        // G is a power of two (cp_create): a runtime division per
+                                                         // unrolled column made the per-item code tens of KB of SASS
     const int R = it.q_tokens * G;                       // <= RC
     const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
     const int tok0 = p.meta.cu_q[it.req] + it.q_start;
@@ -690,7 +702,7 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
         const int r = id >> 4, c = id & 15;
         uint4 v = make_uint4(0, 0, 0, 0);
         if (r < R) {
-            const int tok = tok0 + r / G, head = it.kv_head * G + r % G;
+            const int tok = tok0 + (r >> gs), head = it.kv_head * G + (r & (G - 1));
             v = *reinterpret_cast<const uint4*>(p.q + ((int64_t)tok * sh.Hq + head) * D + c * 8);
         }
         *reinterpret_cast<uint4*>(small + (c >> 3) * 2048 + r * 128 + (((c & 7) ^ (r & 7)) << 4)) = v;
@@ -704,7 +716,7 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
     for (int c = 0; c < RC; ++c) {
         m_ref[c] = -INFINITY;
         l_part[c] = 0.f;
-        limit[c] = c < R ? min(it.kv_end, ctx + it.q_start + c / G + 1) : 0;
+        limit[c] = c < R ? min(it.kv_end, ctx + it.q_start + (c >> gs) + 1) : 0;
     }
     const uint32_t t_row = tmem + (lane_base << 16);
     // P^T element (col c, key `row`): B operand [16 rows][128 keys], K-major, halves (64 keys) 2 KB apart
@@ -793,8 +805,8 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
         if (c < R) {
             const float lc = ls->lsum[0][c] + ls->lsum[1][c] + ls->lsum[2][c] + ls->lsum[3][c];
             if (it.partial_row < 0) {
-                const int tok = tok0 + c / G, head = it.kv_head * G + c % G;
-                p.out[((int64_t)tok * sh.Hq + head) * D + row] = __float2bfloat16_rn(__uint_as_float(o[c]) / lc);
+                const int tok = tok0 + (c >> gs), head = it.kv_head * G + (c & (G - 1));
+                p.out[((int64_t)tok * sh.Hq + head) * D + row] = __float2bfloat16_rn(__fdividef(__uint_as_float(o[c]), lc));
             } else {
                 p.part_o[((int64_t)it.partial_row + c) * D + row] = __uint_as_float(o[c]);
                 if (row == c) p.part_ml[(int64_t)it.partial_row + c] = make_float2(m_ref[c], lc);
@@ -894,8 +906,7 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     // their share to the tile softmax (a 128-column score row in registers) and the decode softmax.
     if (warp < 8) {
         reg_dec<56>();
-        if (warp < kProdT) producer<D, 0>(p, &tmap, smem, &misc->lane[0], lane, warp);
-        else if (warp < kProdT + kProdS) producer<D, 1>(p, &tmap, smem, &misc->lane[1], lane, warp - kProdT);
+        if (warp < kProdT + kProdS) producer<D>(p, &tmap, smem, misc, lane, warp);
         else if (warp == 5) mma_warp<D, 0, 1>(ptx::smem_u32(smem), misc, lane);      // lane T: score blocks (and swap items)
         else if (warp == 6) mma_warp<D, 0, 2>(ptx::smem_u32(smem), misc, lane);      // lane T: PV blocks
         else mma_warp<D, 1, 0>(ptx::smem_u32(smem), misc, lane);                     // lane S
