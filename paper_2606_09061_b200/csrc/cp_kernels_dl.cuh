@@ -336,10 +336,11 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
             const uint32_t k_half = kv_base + slot * L::kSlotBytes + h * 8 * L::kGroupBytes;   // rows 64 h .. 64 h + 63
             const uint32_t d_tmem = tmem + buf * 64;
             if (ptx::elect_one()) {
+                const uint64_t k_desc0 = ptx::umma_desc_sw128(k_half, 16, L::kGroupBytes);
 #pragma unroll
                 for (int ks = 0; ks < D / 16; ++ks) {
                     const uint32_t koff = (ks >> 2) * 1024 + (ks & 3) * 32;            // K slot: halves of D 1 KB apart
-                    umma_ts(d_tmem, tmem + kColQ + ks * 8, ptx::umma_desc_sw128(k_half + koff, 16, L::kGroupBytes), idesc_qk, ks > 0);
+                    umma_ts(d_tmem, tmem + kColQ + ks * 8, ptx::umma_desc_advance(k_desc0, koff), idesc_qk, ks > 0);
                 }
                 if (last_of_slot) ptx::umma_commit(&ls->kv_empty[slot]);
                 ptx::umma_commit(&ls->ts_full[buf]);
@@ -361,10 +362,11 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
             const uint32_t v_half = kv_base + slot * L::kSlotBytes + h * 4 * L::kPageBytes;     // keys 64 h .. 64 h + 63
             const uint32_t d_tmem = tmem + col_o(0);
             if (ptx::elect_one()) {
+                const uint64_t v_desc0 = ptx::umma_desc_sw128(v_half, 1024, L::kGroupBytes);
 #pragma unroll
                 for (int ks = 0; ks < 4; ++ks) {
                     // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
-                    umma_ts(d_tmem, tmem + buf * 64 + ks * 8, ptx::umma_desc_sw128(v_half + ks * L::kPageBytes, 1024, L::kGroupBytes),
+                    umma_ts(d_tmem, tmem + buf * 64 + ks * 8, ptx::umma_desc_advance(v_desc0, ks * L::kPageBytes),
                             idesc_pv, j > 0 || ks > 0);
                 }
                 if (last_of_slot) ptx::umma_commit(&ls->kv_empty[slot]);
@@ -427,6 +429,8 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
         const uint32_t k_tile = kv_base + slot * L::kSlotBytes;
         const uint32_t d_tmem = tmem + col_s(LANE, buf);
         if (ptx::elect_one()) {
+            const uint64_t k_desc0 = ptx::umma_desc_sw128(k_tile, 16, L::kGroupBytes);
+            const uint64_t q_desc0 = ptx::umma_desc_sw128(small, 16, 1024);
 #pragma unroll
 #ifdef DL_X_S_NOMMA
             for (int ks = 0; ks < (swap ? 0 : D / 16); ++ks) {
@@ -434,12 +438,12 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
             for (int ks = 0; ks < D / 16; ++ks) {
 #endif
                 const uint32_t koff = (ks >> 2) * 1024 + (ks & 3) * 32;                // K slot: halves 1 KB apart
-                const uint64_t k_desc = ptx::umma_desc_sw128(k_tile + koff, 16, L::kGroupBytes);
+                const uint64_t k_desc = ptx::umma_desc_advance(k_desc0, koff);
                 if (LANE == 0 && !swap) {
                     umma_ts(d_tmem, tmem + kColQ + ks * 8, k_desc, idesc_qk, ks > 0);
                 } else {
                     const uint32_t qoff = (ks >> 2) * small_half + (ks & 3) * 32;
-                    ptx::umma_ss(d_tmem, k_desc, ptx::umma_desc_sw128(small + qoff, 16, 1024), idesc_qk, ks > 0);
+                    ptx::umma_ss(d_tmem, k_desc, ptx::umma_desc_advance(q_desc0, qoff), idesc_qk, ks > 0);
                 }
             }
             ptx::umma_commit(&ls->kv_empty[slot]);
@@ -461,6 +465,8 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
         const uint32_t v_tile = kv_base + slot * L::kSlotBytes;
         const uint32_t d_tmem = tmem + col_o(LANE);
         if (ptx::elect_one()) {
+            const uint64_t v_desc0 = ptx::umma_desc_sw128(v_tile, 1024, L::kGroupBytes);
+            const uint64_t p_desc0 = ptx::umma_desc_sw128(small + 4096 + buf * 4096, 16, 1024);      // P^T is double buffered
 #pragma unroll
 #ifdef DL_X_S_NOMMA
             for (int ks = 0; ks < (swap ? 0 : kKeyTile / 16); ++ks) {
@@ -468,12 +474,12 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
             for (int ks = 0; ks < kKeyTile / 16; ++ks) {
 #endif
                 // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
-                const uint64_t v_desc = ptx::umma_desc_sw128(v_tile + ks * L::kPageBytes, 1024, L::kGroupBytes);
+                const uint64_t v_desc = ptx::umma_desc_advance(v_desc0, ks * L::kPageBytes);
                 if (LANE == 0 && !swap) {
                     umma_ts(d_tmem, tmem + col_s(0, buf) + ks * 8, v_desc, idesc_pv, t > 0 || ks > 0);
                 } else {
-                    const uint32_t poff = 4096 + buf * 4096 + (ks >> 2) * small_half + (ks & 3) * 32;   // P^T is double buffered
-                    ptx::umma_ss(d_tmem, v_desc, ptx::umma_desc_sw128(small + poff, 16, 1024), idesc_pv, t > 0 || ks > 0);
+                    const uint32_t poff = (ks >> 2) * small_half + (ks & 3) * 32;
+                    ptx::umma_ss(d_tmem, v_desc, ptx::umma_desc_advance(p_desc0, poff), idesc_pv, t > 0 || ks > 0);
                 }
             }
             ptx::umma_commit(&ls->kv_empty[slot]);

@@ -215,6 +215,13 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr, uint32_t
     d |= (uint64_t)2 << 61;        // SWIZZLE_128B
     return d;
 }
+// The same descriptor `bytes` further into shared memory: the start-address field is the low 14 bits
+// (address >> 4) and a tile never crosses the 256 KB it can express, so one add on the low word does it
+// (building every descriptor from scratch cost 4-5 uniform-pipe instructions per MMA operand; the issue
+// loops are part of the hot instruction footprint).
+__device__ __forceinline__ uint64_t umma_desc_advance(uint64_t desc, uint32_t bytes) {
+    return desc + (uint64_t)(bytes >> 4);
+}
 // Instruction descriptor, kind::f16: bf16 x bf16 -> fp32.
 __host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N, bool a_mn_major, bool b_mn_major) {
     return (1u << 4)                       // D format: F32
