@@ -60,7 +60,7 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 #endif
     return ok != 0;
 }
-// A wait that does not complete within ~4 s is a protocol bug: trap (the launch fails with an
+// A wait that does not complete within 2^20 suspended tries (~1-20 s) is a protocol bug: trap (the launch fails with an
 // error) instead of hanging the device.  The default build keeps the wait loop free of function
 // calls (an ABI call anywhere in the kernel stops ptxas from giving the warpgroups the register
 // counts they ask for with setmaxnreg); -DCP_WAIT_DIAG prints which barrier timed out.
@@ -76,17 +76,22 @@ __device__ __noinline__ void mbar_wait_slow(uint64_t* bar, uint32_t parity) {
     }
 }
 #endif
+// The default wait is ONE loop with a spin counter: the earlier form (a first try, then a loop with
+// clock64 arithmetic) was 20 SASS instructions per wait site, and there are ~50 sites inlined into the
+// per-tile loops of every role -- several KB of the 32 KB instruction-cache budget.  A try
+// suspends for up to CP_WAIT_HINT_NS, so the limit is reached after ~1 s (early wake-ups) to ~20 s.
+constexpr uint32_t kWaitSpinLimit = CP_WAIT_HINT_NS >= 4000 ? (1u << 20) : (CP_WAIT_HINT_NS > 0 ? (1u << 24) : (1u << 28));
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    if (mbar_try_wait(bar, parity)) return;
 #ifdef CP_WAIT_DIAG
+    if (mbar_try_wait(bar, parity)) return;
     mbar_wait_slow(bar, parity);
 #else
-    const long long t0 = clock64();
+    uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
 #ifdef DL_X_NANOSLEEP
         __nanosleep(DL_X_NANOSLEEP);
 #endif
-        if (clock64() - t0 > 8000000000LL) __trap();
+        if (++spins > kWaitSpinLimit) __trap();
     }
 #endif
 }
