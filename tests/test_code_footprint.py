@@ -1,0 +1,39 @@
+"""Guard on the instruction footprint of the dual-lane attention kernel (no GPU: reads the SASS of the
+built libcp.so with cuobjdump).
+
+DESIGN.md 7.0: seven warp roles of `dl::attn_dl_kernel` run different code at once against the SM's 32 KB
+L1.5 instruction cache; at 19,216 SASS instructions (a `producer` copy per lane, runtime divisions by the
+GQA group size in column-unrolled code) a mixed batch spent 27 % of its issue slots waiting for instruction
+fetch and ran 1.4x slower.  The kernel is 14,632 instructions now; this test fails if it grows back.
+"""
+import re
+import shutil
+import subprocess
+
+import pytest
+
+from paper_2606_09061_b200 import build
+
+BUDGET = {"attn_dl_kernelILi128E": 15500, "attn_dl_kernelILi64E": 4200}
+
+
+@pytest.mark.skipif(shutil.which("cuobjdump") is None, reason="cuobjdump not on PATH")
+def test_dual_lane_kernel_sass_size_within_budget():
+    lib = build.build()
+    sass = subprocess.run(["cuobjdump", "-sass", lib], check=True, capture_output=True, text=True).stdout
+    counts, cur = {}, None
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            continue
+        if cur and re.match(r"\s+/\*[0-9a-f]{4}\*/\s+\S", line):
+            counts[cur] = counts.get(cur, 0) + 1
+    for key, limit in BUDGET.items():
+        hits = {k: v for k, v in counts.items() if key in k}
+        assert len(hits) == 1, (key, list(counts))
+        (name, n), = hits.items()
+        assert 1000 < n <= limit, f"{name}: {n} SASS instructions > budget {limit} (DESIGN.md 7.0)"
+        # runtime integer division shows up as a call-free reciprocal sequence with I2F.U32.RP: none in the kernel
+    body = sass.split("attn_dl_kernelILi128E", 1)[1].split("Function :", 1)[0]
+    assert body.count("I2F.U32.RP") <= 4, "runtime integer divisions crept back into the per-item code"
