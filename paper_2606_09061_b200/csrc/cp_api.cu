@@ -98,6 +98,7 @@ struct cp_ctx {
     float mem_stats[4] = {0, 0, 0, 0};
     int32_t n_prefill = 0, n_decode = 0;
     int32_t combine_rows = 0;          // rows (token, head) that have split partials to merge
+    bool tensor_bound = false;         // algorithmic FLOPs / 2.25 PF/s > algorithmic bytes / 8 TB/s (nominal B200)
 
     // latency ring
     std::vector<TimedStep> ring;
@@ -233,6 +234,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     int64_t T = 0, P = 0, total_tiles[2] = {0, 0};      // key tiles per item kind (tile, swap)
     float f_pf_tokens = 0, f_dec = 0, f_sum_ctx = 0, f_max_ctx = 0, f_pf_proc = 0, f_pf_proc_max = 0;
     int32_t n_prefill = 0, n_decode = 0;
+    double alg_pairs = 0, alg_keys = 0;
     for (int j = 0; j < n_reqs; ++j) {
         const cp_req_desc& r = reqs[j];
         if (r.q_len < 1 || r.ctx_off < 0 || r.n_blocks < 0 || (!r.block_table && r.n_blocks > 0)) {
@@ -240,6 +242,8 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
             return CP_EINVAL;
         }
         const int64_t kv_len = (int64_t)r.ctx_off + r.q_len;
+        alg_pairs += (double)r.q_len * r.ctx_off + 0.5 * r.q_len * ((double)r.q_len + 1);   // causal (query, key) pairs
+        alg_keys += (double)kv_len;
         if ((int64_t)r.n_blocks * B < kv_len || kv_len > INT32_MAX) {
             cp_set_error("cp_build_batch: request %d: block table covers %lld < %lld tokens", j,
                          (long long)r.n_blocks * B, (long long)kv_len);
@@ -436,6 +440,11 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     c->feat[4] = f_max_ctx; c->feat[5] = f_pf_proc; c->feat[6] = f_pf_proc_max;
     c->n_prefill = n_prefill;
     c->n_decode = n_decode;
+    {   // SURVEY.md 8(d) formulas: FLOPs = 4 D Hq pairs; bytes = KV once per request and KV head + Q + out
+        const double flops = 4.0 * sh.D * sh.Hq * alg_pairs;
+        const double bytes = 2.0 * alg_keys * sh.Hkv * sh.D * 2 + 2.0 * (double)T * sh.Hq * sh.D * 2;
+        c->tensor_bound = flops / 2.25e15 > bytes / 8e12;
+    }
     c->have_batch = true;
     ++c->iter;
     if (c->d_rope_cs && T > 0) {       // positions changed: (cos, sin) table of this batch, same stream as the copy
@@ -545,14 +554,17 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
     if (rc != CP_OK) return rc;
     if (!c->tc_attr_set) {
         CP_CUDA(cudaFuncSetAttribute(attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcLayout<D>::kTotal));
-        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D>::kTotal));
+        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D>::kTotal));
+        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D>::kTotal));
         c->tc_attr_set = true;
     }
     if (m.n_work > 0) {
         const int grid = std::min(c->n_sm, m.n_work);
         if (c->use_dl) {
             dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
-            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D>, dim3(grid), dim3(dl::kThreads), dl::Layout<D>::kTotal, stream, p, *tmap));
+            // tensor-bound batches take the instantiation that moves a quarter of the exponentials to the FMA pipe
+            CP_CUDA(launch_pdl(c->tensor_bound ? dl::attn_dl_kernel<D, true> : dl::attn_dl_kernel<D, false>, dim3(grid),
+                               dim3(dl::kThreads), dl::Layout<D>::kTotal, stream, p, *tmap));
         } else {
             TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
             attn_tc_kernel<D><<<grid, kTcThreads, TcLayout<D>::kTotal, stream>>>(p, *tmap);

@@ -53,10 +53,12 @@ __host__ __device__ constexpr uint32_t col_s(int lane, uint32_t buf) { return la
 __host__ __device__ constexpr uint32_t col_o(int lane) { return lane == 0 ? 256u : 480u; }
 constexpr uint32_t kColQ = 384;
 #ifndef DL_POLY_EVERY
-#define DL_POLY_EVERY 0
+#define DL_POLY_EVERY 4
 #endif
-// tile kind: every kPolyEvery-th exponential runs on the FMA pipe (0 = none).  Measured on B200: 4 -> -3.5 % on
-// chunk-only batches, +3 % on the mixed batch (the extra FMA-pipe instructions compete with the decode lane): off.
+// tile kind: in the POLY instantiation of the kernel every kPolyEvery-th exponential runs on the FMA pipe.
+// Measured on B200 (final kernel): 4 -> -3.5 % on chunk-only batches, -2 % on the 70B-shaped chunk, +1 % on the
+// mixed batch of configs[2] (HBM-bound: the exponentials are not its limit and the extra FMA-pipe instructions
+// are).  The host therefore picks the instantiation per batch: POLY for tensor-bound batches only (cp_api.cu).
 constexpr int kPolyEvery = DL_POLY_EVERY;
 constexpr float kRescaleThreshold = 8.0f;      // log2 units: rescale O only when the max grew > 2^8
 constexpr uint32_t kSmallBytes = 12288;        // per lane: Q^T (4 KiB) + double-buffered P^T (8 KiB)
@@ -138,8 +140,9 @@ struct Params {
 };
 
 // element e of a half-tile row: MUFU or FMA-pipe exponential (e is a constant after unrolling)
+template <bool POLY>
 __device__ __forceinline__ float ex2_sel(float x, int e) {
-    return (kPolyEvery > 0 && e % (kPolyEvery > 0 ? kPolyEvery : 1) == (kPolyEvery > 0 ? kPolyEvery : 1) - 1) ? ptx::ex2_poly(x) : ptx::ex2(x);
+    return (POLY && kPolyEvery > 0 && e % (kPolyEvery > 0 ? kPolyEvery : 1) == (kPolyEvery > 0 ? kPolyEvery : 1) - 1) ? ptx::ex2_poly(x) : ptx::ex2(x);
 }
 
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
@@ -527,7 +530,7 @@ __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lan
 // tile), online softmax (log2 domain, lazy rescale), P row -> TMEM over the first 64 columns of the
 // same S buffer (bf16 pairs), O rescale / epilogue from TMEM.
 // ------------------------------------------------------------------------------------------
-template <int D>
+template <int D, bool POLY>
 __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p, LaneState* ls, uint32_t tmem,
                                              uint32_t& gh, int row, uint32_t lane_base) {
     const Shape& sh = p.sh;
@@ -614,16 +617,16 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         if (nvalid == 64) {
 #pragma unroll
             for (int i = 0; i < 64; i += 2) {
-                const float a = ex2_sel(fmaf(__uint_as_float(sr[i]), scale, neg_m), i);
-                const float b = ex2_sel(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1);
+                const float a = ex2_sel<POLY>(fmaf(__uint_as_float(sr[i]), scale, neg_m), i);
+                const float b = ex2_sel<POLY>(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1);
                 sm[(i >> 1) & 3] += a + b;
                 pk[i >> 1] = pack_bf16(a, b);
             }
         } else {
 #pragma unroll
             for (int i = 0; i < 64; i += 2) {
-                const float a = i < nvalid ? ex2_sel(fmaf(__uint_as_float(sr[i]), scale, neg_m), i) : 0.f;
-                const float b = i + 1 < nvalid ? ex2_sel(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1) : 0.f;
+                const float a = i < nvalid ? ex2_sel<POLY>(fmaf(__uint_as_float(sr[i]), scale, neg_m), i) : 0.f;
+                const float b = i + 1 < nvalid ? ex2_sel<POLY>(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1) : 0.f;
                 sm[(i >> 1) & 3] += a + b;
                 pk[i >> 1] = pack_bf16(a, b);
             }
@@ -825,7 +828,7 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
 
 // softmax warpgroup loop.  ROLE 0: lane T (tile kind, and the swap-kind items lane T picks up);
 // ROLE 2: lane S.
-template <int D, int ROLE>
+template <int D, int ROLE, bool POLY>
 __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Misc* misc, int warp, int lane) {
     using L = Layout<D>;
     constexpr int LANE = ROLE == 2 ? 1 : 0;
@@ -849,7 +852,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
                 else softmax_swap<LANE, 16>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
             }
         } else {
-            if constexpr (ROLE == 0) softmax_tile<D>(it, p, ls, tmem, gh_tile, row, lane_base);
+            if constexpr (ROLE == 0) softmax_tile<D, POLY>(it, p, ls, tmem, gh_tile, row, lane_base);
         }
         ++item_cnt;
     }
@@ -858,7 +861,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
 // ------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------
-template <int D>
+template <int D, bool POLY>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     using L = Layout<D>;
@@ -918,10 +921,10 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         else mma_warp<D, 1, 0>(ptx::smem_u32(smem), misc, lane);                     // lane S
     } else if (warp < 12) {
         reg_inc<232>();
-        softmax_warps<D, 0>(p, smem, misc, warp, lane);
+        softmax_warps<D, 0, POLY>(p, smem, misc, warp, lane);
     } else {
         reg_inc<160>();
-        softmax_warps<D, 2>(p, smem, misc, warp, lane);
+        softmax_warps<D, 2, false>(p, smem, misc, warp, lane);
     }
     ptx::tc_fence_before();
     __syncthreads();

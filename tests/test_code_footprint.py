@@ -31,9 +31,9 @@ def test_dual_lane_kernel_sass_size_within_budget():
             counts[cur] = counts.get(cur, 0) + 1
     for key, limit in BUDGET.items():
         hits = {k: v for k, v in counts.items() if key in k}
-        assert len(hits) == 1, (key, list(counts))
-        (name, n), = hits.items()
-        assert 1000 < n <= limit, f"{name}: {n} SASS instructions > budget {limit} (DESIGN.md 7.0)"
-        # runtime integer division shows up as a call-free reciprocal sequence with I2F.U32.RP: none in the kernel
-    body = sass.split("attn_dl_kernelILi128E", 1)[1].split("Function :", 1)[0]
-    assert body.count("I2F.U32.RP") <= 4, "runtime integer divisions crept back into the per-item code"
+        assert len(hits) == 2, (key, list(counts))        # the MUFU-only and the FMA-pipe-share instantiation
+        for name, n in hits.items():
+            assert 1000 < n <= limit, f"{name}: {n} SASS instructions > budget {limit} (DESIGN.md 7.0)"
+    # a runtime integer division shows up as a reciprocal sequence starting with I2F.U32.RP
+    for body in sass.split("attn_dl_kernelILi128E")[1:]:
+        assert body.split("Function :", 1)[0].count("I2F.U32.RP") <= 4, "runtime integer divisions crept back"

@@ -243,3 +243,27 @@ def test_repeated_launches_mixed_shapes_no_deadlock():
         got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)[tok, head]
         gu.assert_close(got, want, spec.name)
     ctx.close()
+
+
+@pytest.mark.parametrize("Hq,Hkv,D,q_len,ctx_off", [(8, 2, 128, [300, 129], [517, 0]), (8, 2, 64, [257], [1000]),
+                                                    (32, 8, 128, [384], [2048])])
+def test_tensor_bound_batches_take_the_fma_pipe_share_kernel(Hq, Hkv, D, q_len, ctx_off):
+    """Chunk-only batches are tensor-bound by the SURVEY.md 8(d) formulas, so cp_attention_step launches the
+    instantiation that evaluates every fourth exponential of a score row with a polynomial on the FMA pipe
+    (DESIGN.md 6.1); same tolerance, full oracle.  The same chunks next to long decodes form an HBM-bound batch
+    and take the MUFU-only instantiation: also within tolerance."""
+    pages = sum((q + o + 15) // 16 for q, o in zip(q_len, ctx_off)) + 40
+    spec = wl.make_spec("tensor_bound", Hq, Hkv, D, 16, pages, q_len, ctx_off, seed=21)
+    hv = wl.host_values(spec)
+    got, _ = gu.run_gpu_host_values(spec, hv, 0)
+    want, _ = gu.run_oracle_host_values(spec, hv)
+    gu.assert_close(got, want, "tensor-bound batch")
+    # the same chunks next to enough long decodes to make the batch HBM-bound: the MUFU-only instantiation
+    dec_ctx = [6000] * 24
+    spec2 = wl.make_spec("hbm_bound", Hq, Hkv, D, 16, pages + 24 * 376 + 40, q_len + [1] * 24,
+                         ctx_off + [c - 1 for c in dec_ctx], seed=21)
+    hv2 = wl.host_values(spec2)
+    got2, _ = gu.run_gpu_host_values(spec2, hv2, 0)
+    tok, head = gu.sample_rows(spec2, 256, seed=3)
+    want2, _ = gu.run_oracle_host_values(spec2, hv2, rows=(tok, head))
+    gu.assert_close(got2[tok, head], want2, "hbm-bound batch")
