@@ -137,12 +137,27 @@ def oracle_sample_rate(spec, q_bits, cache_bits, target_s, seed=0):
 
 def ncu_traffic(workload):
     """DRAM bytes per launch of the attention kernel from the committed `ncu --set full` capture of this
-    workload (profiles/traffic.json, written by hand from the capture named there); None if not captured."""
+    workload (profiles/traffic.json: a STATIC figure copied from the capture named there, not measured in
+    this run -- it goes stale when the kernel or the work-list order changes, hence the source string that
+    travels with it).  Returns (bytes or None, source or None)."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     try:
-        return json.load(open(p)).get(workload, {}).get("dram_bytes_per_launch")
+        e = json.load(open(p)).get(workload, {})
+        if "dram_bytes_per_launch" not in e:
+            return None, None
+        return e["dram_bytes_per_launch"], f"profiles/traffic.json (static; {e.get('capture', 'capture unnamed')}; kernel at commit {e.get('commit', '?')})"
     except Exception:
-        return None
+        return None, None
+
+
+def config_dict(spec, kv_dtype="bf16"):
+    """The workload description, identical in both arms (ours and --impl reference)."""
+    return {"workload": f"BASELINE.json configs[2] '{spec.name}'" if spec.name == "b2048" else spec.name,
+            "tokens": spec.T, "requests": spec.n_reqs, "decodes": int((spec.q_len == 1).sum()),
+            "prefill_chunks": int((spec.q_len > 1).sum()), "sum_kv_len": int(spec.kv_len.sum()),
+            "pages": int(sum(len(b) for b in spec.block_tables)), "pool_pages": spec.num_blocks,
+            "Hq": spec.Hq, "Hkv": spec.Hkv, "D": spec.D, "block": spec.B, "layers_per_step": 1,
+            "kv_dtype": kv_dtype, "l2": "inputs_exceed_l2 (KV >> 126 MB), no flush"}
 
 
 def dist_env():
@@ -180,7 +195,7 @@ def run_ours(args):
     n_pages = int(sum(len(b) for b in spec.block_tables))
     ctx = binding.Context(spec.Hq, spec.Hkv, spec.D, spec.num_blocks, spec.B, sm_scale=spec.sm_scale,
                           max_tokens=spec.T, max_reqs=spec.n_reqs, max_total_pages=n_pages,
-                          device=local_rank, kernel_variant=args.variant)
+                          device=local_rank)
     descs, keep = binding.make_descs(spec.q_len, spec.ctx_off, spec.block_tables)
     out = torch.empty((spec.T, spec.Hq, spec.D), device=dev, dtype=torch.bfloat16)
     free_b, total_b = torch.cuda.mem_get_info(dev)
@@ -294,23 +309,25 @@ def run_ours(args):
     attn_us = float(np.mean(step_us)) if len(step_us) else ms_per_step * 1e3
     bytes_alg, flops_alg = spec.algorithmic_bytes(), spec.flops()
     t_hbm = bytes_alg / (peaks["hbm_gbs"] * 1e9)
-    t_tc = flops_alg / (peaks["bf16_tflops_sustained"] * 1e12)
+    # the tensor peak that applies (B200_PROFILING.md): the burst figure for a kernel timed alone for a short while,
+    # the sustained one when the timed region is long enough for the power cap to engage (>= 1 s, or sw_power_cap seen)
+    sustained = ms_total >= 1000.0 or "sw_power_cap" in (clocks.get("reasons") or [])
+    tc_peak = peaks["bf16_tflops_sustained"] if sustained else peaks["bf16_tflops"]
+    t_tc = flops_alg / (tc_peak * 1e12)
     bound = "hbm" if t_hbm >= t_tc else "tensor"
     if bound == "hbm":
         achieved, peak, runit = bytes_alg / (attn_us * 1e-6) / 1e9, peaks["hbm_gbs"], "GB/s"
     else:
-        achieved, peak, runit = flops_alg / (attn_us * 1e-6) / 1e12, peaks["bf16_tflops_sustained"], "TFLOP/s"
+        achieved, peak, runit = flops_alg / (attn_us * 1e-6) / 1e12, tc_peak, "TFLOP/s"
+    traffic, traffic_source = ncu_traffic(spec.name)
     res = {
         "metric": METRIC, "value": tokens_per_s, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[2] '{spec.name}'" if spec.name == "b2048" else spec.name,
-                   "tokens": spec.T, "requests": spec.n_reqs, "decodes": int((spec.q_len == 1).sum()),
-                   "prefill_chunks": int((spec.q_len > 1).sum()), "sum_kv_len": int(spec.kv_len.sum()),
-                   "pages": n_pages, "pool_pages": spec.num_blocks, "Hq": spec.Hq, "Hkv": spec.Hkv,
-                   "D": spec.D, "block": spec.B, "layers_per_step": 1, "l2": "inputs_exceed_l2 (KV >> 126 MB), no flush",
-                   "parallelism": "replicas" if world > 1 else "single", "kernel_variant": args.variant, "rope": bool(args.rope),
-                   "work_items": info.n_work_items, "combine_items": info.n_combine_items},
+        "config": config_dict(spec),
+        "launch": {"parallelism": "replicas" if world > 1 else "single", "rope": bool(args.rope),
+                   "work_items": info.n_work_items, "combine_items": info.n_combine_items,
+                   "grid_attn": info.grid_attn, "kernels_per_step": info.kernels_per_step},
         "clocks": clocks,
         "e2e": {"value": whole_job_rate(spec.T, args.steps, world, e2e_ms), "unit": UNIT,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps},
@@ -325,7 +342,11 @@ def run_ours(args):
                          "build_batch_host_median": build_batch_us, "build_batch_h2d_bytes": int(meta_bytes)},
         "tflops": flops_alg / (attn_us * 1e-6) / 1e12, "gbs": bytes_alg / (attn_us * 1e-6) / 1e9,
         "roofline": {"bound": bound, "achieved": achieved, "peak": peak, "unit": runit,
-                     "frac": achieved / peak, "traffic": ncu_traffic(spec.name) if args.variant == 0 else None, "peak_source": peaks["source"],
+                     "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source,
+                     "peak_source": peaks["source"] + (" (sustained)" if bound == "tensor" and sustained else " (burst)" if bound == "tensor" else ""),
+                     "frac_of_tensor_burst": flops_alg / (attn_us * 1e-6) / 1e12 / peaks["bf16_tflops"],
+                     "frac_of_tensor_sustained": flops_alg / (attn_us * 1e-6) / 1e12 / peaks["bf16_tflops_sustained"],
+                     "frac_of_hbm": bytes_alg / (attn_us * 1e-6) / 1e9 / peaks["hbm_gbs"],
                      "kernel": "cp_attention_step kernels (append + attention + combine), mean of CUDA-event pairs",
                      "algorithmic_bytes": bytes_alg, "algorithmic_flops": flops_alg,
                      "t_hbm_us": t_hbm * 1e6, "t_tensor_us": t_tc * 1e6,
@@ -363,17 +384,26 @@ def run_reference(args):
         hv = wl.host_values(spec)
         qb, kb, vb, cache = hv.q, hv.k_new, hv.v_new, hv.cache
     ora.kv_append(kb, vb, cache, spec.q_len, spec.ctx_off, spec.compact_tables())
-    per_step_s = max(1.0, min(20.0, 120.0 / (args.steps + args.warmup)))
-    vals, descs, threads = [], [], 1
-    for i in range(args.warmup + args.steps):
+    # A step = the oracle over the WHOLE batch when warm-up + steps of that fit ~5 minutes on this host (configs[2]:
+    # ~7 s per step on 16 cores); otherwise a bounded seeded row sample per step, the full-batch rate extrapolated by
+    # the causal-pair ratio and the line says so ("extrapolated": true; ms_per_step stays the measured wall time).
+    n_steps = args.warmup + args.steps
+    v0, threads, _ = oracle_sample_rate(spec, qb, cache, 1.0, seed=10_000)
+    full_s = spec.T / v0
+    whole = full_s * n_steps <= 300.0
+    per_step_s = 1e9 if whole else max(1.0, min(20.0, 150.0 / n_steps))
+    vals, descs, walls = [], [], []
+    for i in range(n_steps):
+        t0 = time.perf_counter()
         v, threads, desc = oracle_sample_rate(spec, qb, cache, per_step_s, seed=i)
         if i >= args.warmup:
-            vals.append(v); descs.append(desc)
+            vals.append(v); descs.append(desc); walls.append(time.perf_counter() - t0)
     v = float(np.mean(vals))
     res = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world,
-           "steps": args.steps, "warmup": args.warmup, "ms_per_step": spec.T / v * 1e3,
+           "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": spec.T / v * 1e3 if whole else float(np.mean(walls)) * 1e3, "extrapolated": not whole,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-           "data": "synthetic", "config": {"workload": spec.name, "tokens": spec.T, "requests": spec.n_reqs},
+           "data": "synthetic", "config": config_dict(spec),
            "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": descs[-1]},
            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(res), flush=True)
@@ -386,12 +416,18 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="b2048", choices=sorted(wl.CONFIGS))
-    ap.add_argument("--variant", type=int, default=0, help="cp_config.kernel_variant")
     ap.add_argument("--rope", action="store_true",
                     help="time cp_attention_step_rope (rotary embedding of Q / new K fused into the append)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.gpus > 1 and "RANK" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: re-exec under torch.distributed.run, one replica per GPU
+        # (rendezvous on 127.0.0.1; "replicas only")
+        port = 29500 + os.getpid() % 2000
+        os.execvp(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                   f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+                                   "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]])
     if args.impl == "reference":
         run_reference(args)
     else:

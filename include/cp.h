@@ -9,10 +9,11 @@
  *
  * Ownership: the caller owns every device tensor it passes (q, k_new, v_new, kv_cache,
  * out) and the CUDA stream.  The library owns its context, device metadata, the
- * split-KV partial workspace, pinned staging and CUDA events, all allocated in
- * cp_create from the limits in cp_config; nothing is allocated and nothing
- * synchronises afterwards, except cp_latency_table (may wait on the newest timed
- * step) and cp_destroy.
+ * split-KV partial workspace, pinned staging, a copy stream and CUDA events, all
+ * allocated in cp_create from the limits in cp_config; nothing is allocated afterwards.
+ * Calls that may block the host: cp_latency_table (waits for the newest timed step),
+ * cp_destroy, cp_enable_rope, and cp_build_batch ONLY when the host runs more than three
+ * batches ahead of the device (the metadata staging ring is four batches deep).
  *
  * The operation (PAPER.md:61, :87 chunked-prefill mixed batch; PAPER.md:41 paged KV;
  * defined in DESIGN.md section 2, restating SURVEY.md 8(c1)): for request j, row
@@ -20,7 +21,8 @@
  *     s_t = sm_scale * <q[tok(j,i),h,:], K_j[t,g,:]>,  out = softmax_t(s) . V_j[:,g,:]
  * where K_j[t], V_j[t] live in page block_table_j[t / B], slot t % B.  A decode is
  * simply q_len == 1.  Stale data in page tails / other pages never influences the
- * result (finite stale values; see DESIGN.md for NaN tails).
+ * result, whatever its bit pattern (NaN and Inf included): masked scores are removed by
+ * select and the slots past a request's last key never reach the PV product.
  */
 #ifndef CP_H_
 #define CP_H_
@@ -48,9 +50,7 @@ typedef struct cp_sched cp_sched;   /* opaque */
  *     kv_cache[layer][block][kv: 0 = K, 1 = V][kv_head][slot in 0..B-1][d in 0..D-1]
  * A (block, kv, head) slab is B*D*2 bytes contiguous (4 KiB at B 16, D 128); K and V
  * of a block are adjacent.  cp_attention_step takes the pointer to the LAYER's pool.
- * Pages named by a block table must hold FINITE bf16 values in all their slots, written
- * or not (zero-fill the pool once after allocating it): masked probabilities are exactly
- * 0, but 0 x NaN in the tensor-core PV product would still be NaN.
+ * The pool needs no initialisation (a torch.empty pool is fine).
  * ------------------------------------------------------------------------------- */
 typedef struct {
     int32_t num_q_heads;      /* Hq                                               */
@@ -66,19 +66,25 @@ typedef struct {
     int64_t max_partial_rows; /* split-KV workspace rows ((D+2) fp32 each);
                                  0 = default 4 * max_tokens * Hq                  */
     int32_t device;           /* CUDA device ordinal                              */
-    int32_t kernel_variant;   /* 0 = default: dual-lane tcgen05 kernel (chunk tiles and
-                                     decode streams co-resident on every SM),
-                                 1 = SIMT reference kernels (debug cross-check),
-                                 2 = single-lane tcgen05 kernel (round-1 baseline)   */
+    int32_t kernel_variant;   /* must be 0.  (Library builds with -DCP_DEBUG_VARIANTS also
+                                 accept 1 = a SIMT cross-check kernel for bisecting; the
+                                 shipped library holds one attention kernel and rejects it.) */
 } cp_config;
 
 /* One request of the iteration.  HOST pointers. */
+#define CP_REQ_PREFILL 1         /* flags: this request is in its prefill phase   */
 typedef struct {
     int64_t        req_id;
     int32_t        q_len;        /* >= 1 tokens scheduled this iteration          */
     int32_t        ctx_off;      /* >= 0 tokens already in the cache before them  */
     const int32_t* block_table;  /* HOST: n_blocks page ids in [0, num_blocks)    */
     int32_t        n_blocks;     /* n_blocks * B >= ctx_off + q_len               */
+    int32_t        flags;        /* CP_REQ_PREFILL or 0.  Only the Table-1 features and
+                                    n_prefill / n_decode of cp_latency_row read it: a
+                                    1-token prefill chunk (Eq. 8's candidate c = 1, the last
+                                    token of a prompt) counts as prefill there, as in the
+                                    scheduler's own features.  q_len > 1 is always prefill.
+                                    The computation is the same either way.            */
 } cp_req_desc;
 
 /* One timed step: the 11 raw features of Table 1 + measured us
@@ -89,8 +95,8 @@ typedef struct {
           prefill_processed_tokens, max_prefill_processed_tokens, gpu_mem_used_mb,
           gpu_mem_free_mb, cuda_allocated_mb, cuda_reserved_mb                    */
     float   us;                 /* device time of cp_attention_step (CUDA events)  */
-    int32_t n_prefill;          /* requests with q_len > 1                         */
-    int32_t n_decode;           /* requests with q_len == 1                        */
+    int32_t n_prefill;          /* requests with q_len > 1 or CP_REQ_PREFILL       */
+    int32_t n_decode;           /* the others                                      */
     int32_t layer;
     int64_t iter;               /* index of the cp_build_batch this step ran under */
 } cp_latency_row;
@@ -107,8 +113,13 @@ int cp_destroy(cp_ctx* ctx);
  * host->device copy on `cuda_stream` (a cudaStream_t, may be NULL = default stream).
  * reqs: HOST array of n_reqs descriptors, any mix/order of prefill chunks and decodes;
  * token order of q/out = descriptor order, rows of a request contiguous.
- * A page id may appear in only one request of the batch.  The metadata stays valid for
- * any number of cp_attention_step calls (all layers) until the next cp_build_batch.
+ * A page id may appear in only one request of the batch (no prefix sharing); this is NOT
+ * checked (a duplicate with k_new set is a write race) except in -DCP_DEBUG_VARIANTS
+ * builds, which return CP_EINVAL.  The metadata stays valid for any number of
+ * cp_attention_step calls (all layers) until the next cp_build_batch; its host->device
+ * copy runs on the library's copy stream, overlapping the previous batch's steps, and
+ * `cuda_stream` waits for it.  All steps of a batch must run on one stream (or on
+ * streams the caller orders after it).
  * Errors: CP_EINVAL (q_len < 1, ctx_off < 0, table too short, page id out of range),
  * CP_ECAPACITY (limits of cp_config), CP_ECUDA.  On error the previous batch is kept. */
 int cp_build_batch(cp_ctx* ctx, const cp_req_desc* reqs, int32_t n_reqs,

@@ -16,6 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcp.so")
 
 CP_OK, CP_EINVAL, CP_ECAPACITY, CP_ECUDA, CP_ESTATE = 0, -1, -2, -3, -4
+CP_REQ_PREFILL = 1
 CP_MODE_TOKEN_BUDGET, CP_MODE_LPRS = 0, 1
 CP_PRED_LINEAR, CP_PRED_MLP = 0, 1
 CP_NUM_RAW_FEATURES = 11
@@ -40,7 +41,7 @@ class cp_config(C.Structure):
 
 class cp_req_desc(C.Structure):
     _fields_ = [("req_id", C.c_int64), ("q_len", C.c_int32), ("ctx_off", C.c_int32),
-                ("block_table", C.POINTER(C.c_int32)), ("n_blocks", C.c_int32)]
+                ("block_table", C.POINTER(C.c_int32)), ("n_blocks", C.c_int32), ("flags", C.c_int32)]
 
 
 class cp_latency_row(C.Structure):
@@ -134,7 +135,7 @@ def _check(rc: int):
 
 
 def make_descs(q_len: Sequence[int], ctx_off: Sequence[int], block_tables: Sequence[np.ndarray],
-               req_ids: Optional[Sequence[int]] = None):
+               req_ids: Optional[Sequence[int]] = None, flags: Optional[Sequence[int]] = None):
     """Marshal a batch into a cp_req_desc array (keeps the int32 tables alive)."""
     n = len(q_len)
     arr = (cp_req_desc * max(n, 1))()
@@ -147,6 +148,7 @@ def make_descs(q_len: Sequence[int], ctx_off: Sequence[int], block_tables: Seque
         arr[j].ctx_off = int(ctx_off[j])
         arr[j].block_table = bt.ctypes.data_as(C.POINTER(C.c_int32))
         arr[j].n_blocks = len(bt)
+        arr[j].flags = int(flags[j]) if flags is not None else 0
     return arr, keep
 
 
@@ -180,9 +182,9 @@ class Context:
         self._keep = None
 
     def cp_build_batch(self, q_len=None, ctx_off=None, block_tables=None, stream=None,
-                       descs=None, n=None):
+                       descs=None, n=None, flags=None):
         if descs is None:
-            descs, self._keep = make_descs(q_len, ctx_off, block_tables)
+            descs, self._keep = make_descs(q_len, ctx_off, block_tables, flags=flags)
             n = len(q_len)
         _check(self.lib.cp_build_batch(self.handle, descs, n, _ptr(stream)))
 

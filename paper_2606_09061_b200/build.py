@@ -37,8 +37,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     nv = list(NVCC_FLAGS)
-    if os.path.exists(os.path.join(CSRC, "cp_kernels_tc.cuh")):
-        nv.append("-DCP_WITH_TC")
     if verbose:
         nv += ["-Xptxas", "-v"]
     nv += os.environ.get("CP_EXTRA_NVCC", "").split()

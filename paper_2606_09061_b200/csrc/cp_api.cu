@@ -13,10 +13,7 @@
 
 #include "cp_internal.h"
 #include "cp_kernels_simt.cuh"
-#ifdef CP_WITH_TC
 #include "cp_kernels_dl.cuh"
-#include "cp_kernels_tc.cuh"
-#endif
 
 using namespace cp;
 
@@ -50,6 +47,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 }
 
 constexpr int kRing = 4096;           // timed steps kept for cp_latency_table
+constexpr int kMetaRing = 4;          // batches whose metadata may be in flight (staging + device copies)
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -65,29 +63,32 @@ struct cp_ctx {
     Shape shape{};
     int n_sm = 148;
     int tq = 32;                       // tokens per Q tile = 128 / G
-    bool use_tc = false;               // a tensor-core variant (0 or 2)
-    bool use_dl = false;               // variant 0: the dual-lane kernel
+    bool use_tc = true;                // false only in -DCP_DEBUG_VARIANTS builds with kernel_variant 1 (SIMT cross-check)
 
     // limits
     size_t max_items = 0, max_combine = 0, meta_cap = 0;
     int64_t max_partial_rows = 0;
 
     // device
-    uint8_t* d_meta = nullptr;
+    uint8_t* d_meta[kMetaRing] = {};   // ring: the copy of batch n overlaps the steps of batch n-1
     float* d_part_o = nullptr;
     float2* d_part_ml = nullptr;
     int32_t* d_counter = nullptr;      // persistent-kernel work counter
-    unsigned long long* d_prof = nullptr;   // CP_TC_PROF builds only
     // rotary embedding fused into the append (cp_enable_rope); all null / -1 until enabled
     double* d_inv_freq = nullptr;      // [D/2]
     float2* d_rope_cs = nullptr;       // [max_tokens][D/2] (cos, sin) of the current batch's positions
     __nv_bfloat16* d_q_rot = nullptr;  // [max_tokens][Hq][D] rotated Q of the running step
     int64_t rope_table_iter = -1;      // iter the table was computed for
-    // pinned staging, double buffered
-    uint8_t* h_stage[2] = {nullptr, nullptr};
-    cudaEvent_t stage_done[2] = {nullptr, nullptr};
-    bool stage_used[2] = {false, false};
-    int stage_idx = 0;
+    // pinned staging ring + the library's copy stream.  Slot s = batch number % kMetaRing:
+    //   copy_done[s]  (copy stream)      the H2D of the slot's batch has finished
+    //   batch_end[s]  (caller's stream)  recorded by the NEXT cp_build_batch: every step of the slot's batch precedes it
+    uint8_t* h_stage[kMetaRing] = {};
+    cudaEvent_t copy_done[kMetaRing] = {};
+    cudaEvent_t batch_end[kMetaRing] = {};
+    bool slot_used[kMetaRing] = {};
+    int slot = -1;                     // slot of the current batch
+    cudaStream_t copy_stream = nullptr;
+    cudaStream_t step_stream = nullptr;   // stream of the current batch's most recent step (else of its build)
 
     // current batch
     bool have_batch = false;
@@ -108,6 +109,10 @@ struct cp_ctx {
     std::vector<WorkItem> items, sorted;
     std::vector<CombineItem> combines;
     std::vector<int32_t> bucket, plan, plan_prow;
+#ifdef CP_DEBUG_VARIANTS
+    std::vector<uint32_t> page_mark;   // debug builds: page -> number of the last build that named it
+    uint32_t mark_epoch = 0;
+#endif
 
     // tensor-core path: one TMA descriptor per KV pool pointer (one per layer), encoded once
     std::vector<std::pair<const void*, CUtensorMap>> tmaps;
@@ -126,6 +131,8 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     if (cfg->num_blocks < 1 || cfg->max_tokens < 1 || cfg->max_reqs < 1 || cfg->max_total_pages < 1 ||
         cfg->num_layers < 1) { cp_set_error("cp_create: limits must be positive"); return CP_EINVAL; }
     if ((int64_t)cfg->num_blocks * 2 * Hkv >= (int64_t)1 << 31) { cp_set_error("cp_create: pool too large for 32-bit slab index"); return CP_EINVAL; }
+    // the kernels take max(raw score) * scale as the maximum of the scaled scores
+    if (!(cfg->sm_scale > 0.f) || cfg->sm_scale - cfg->sm_scale != 0.f) { cp_set_error("cp_create: sm_scale must be finite and > 0"); return CP_EINVAL; }
 
     CP_CUDA(cudaSetDevice(cfg->device));
     cp_ctx* c = new cp_ctx();
@@ -134,20 +141,15 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     c->tq = 128 / G;
     cudaDeviceProp prop{};
     if (cudaGetDeviceProperties(&prop, cfg->device) == cudaSuccess) c->n_sm = prop.multiProcessorCount;
-#ifdef CP_WITH_TC
-    c->use_tc = (cfg->kernel_variant == 0 || cfg->kernel_variant == 2) && prop.major == 10;
-    c->use_dl = c->use_tc && cfg->kernel_variant == 0;
+    // ONE attention kernel (no dispatch, no fallback): refuse anything but an sm_100 device.  Debug builds
+    // (-DCP_DEBUG_VARIANTS) additionally accept kernel_variant 1, the SIMT cross-check kernel used for bisecting.
+#ifdef CP_DEBUG_VARIANTS
+    if (cfg->kernel_variant != 0 && cfg->kernel_variant != 1) { delete c; cp_set_error("cp_create: kernel_variant must be 0 or 1"); return CP_EINVAL; }
+    c->use_tc = cfg->kernel_variant == 0;
+#else
+    if (cfg->kernel_variant != 0) { delete c; cp_set_error("cp_create: kernel_variant must be 0 (other values exist only in -DCP_DEBUG_VARIANTS builds)"); return CP_EINVAL; }
 #endif
-    if (cfg->kernel_variant < 0 || cfg->kernel_variant > 2) { delete c; cp_set_error("cp_create: kernel_variant must be 0, 1 or 2"); return CP_EINVAL; }
-    if (cfg->kernel_variant != 1 && !c->use_tc) {
-        // the default variant is the tensor-core path; refuse to run it silently on
-        // something else (no fallback dispatch).  Variant 1 is the explicit SIMT path.
-#ifdef CP_WITH_TC
-        delete c;
-        cp_set_error("cp_create: kernel_variant 0 / 2 need an sm_100 device");
-        return CP_EINVAL;
-#endif
-    }
+    if (c->use_tc && prop.major != 10) { delete c; cp_set_error("cp_create: the attention kernel needs an sm_100 device"); return CP_EINVAL; }
     const size_t q_tiles = (size_t)cfg->max_reqs + (size_t)cfg->max_tokens / c->tq + 1;
     c->max_items = q_tiles * Hkv + (size_t)c->n_sm * 16 + 64;
     c->max_combine = q_tiles * Hkv;
@@ -164,19 +166,17 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
 
     cudaError_t e = cudaSuccess;
     auto chk = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-    chk(cudaMalloc(&c->d_meta, cap));
+    for (int i = 0; i < kMetaRing; ++i) chk(cudaMalloc(&c->d_meta[i], cap));
     chk(cudaMalloc(&c->d_part_o, sizeof(float) * (size_t)c->max_partial_rows * D));
     chk(cudaMalloc(&c->d_part_ml, sizeof(float2) * (size_t)c->max_partial_rows));
     chk(cudaMalloc(&c->d_counter, sizeof(int32_t) * 4));
-#if defined(CP_TC_PROF) || defined(CP_TC_PROF2) || defined(CP_TL)
-    chk(cudaMalloc(&c->d_prof, sizeof(unsigned long long) * 32 * 1024));
-    chk(cudaMemset(c->d_prof, 0, sizeof(unsigned long long) * 32 * 1024));
-#endif
     chk(cudaMemset(c->d_counter, 0, sizeof(int32_t) * 4));
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < kMetaRing; ++i) {
         chk(cudaMallocHost(&c->h_stage[i], cap));
-        chk(cudaEventCreateWithFlags(&c->stage_done[i], cudaEventDisableTiming));
+        chk(cudaEventCreateWithFlags(&c->copy_done[i], cudaEventDisableTiming));
+        chk(cudaEventCreateWithFlags(&c->batch_end[i], cudaEventDisableTiming));
     }
+    chk(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
     c->ring.resize(kRing);
     for (auto& t : c->ring) {
         chk(cudaEventCreate(&t.start));
@@ -187,6 +187,9 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
         cp_destroy(c);
         return CP_ECUDA;
     }
+#ifdef CP_DEBUG_VARIANTS
+    c->page_mark.assign((size_t)cfg->num_blocks, 0);
+#endif
     c->items.reserve(c->max_items);
     c->sorted.reserve(c->max_items);
     c->combines.reserve(c->max_combine);
@@ -200,18 +203,19 @@ extern "C" int cp_destroy(cp_ctx* c) {
     if (!c) return CP_OK;
     cudaSetDevice(c->cfg.device);
     cudaDeviceSynchronize();
-    cudaFree(c->d_meta);
+    for (int i = 0; i < kMetaRing; ++i) cudaFree(c->d_meta[i]);
     cudaFree(c->d_part_o);
     cudaFree(c->d_part_ml);
     cudaFree(c->d_counter);
-    cudaFree(c->d_prof);
     cudaFree(c->d_inv_freq);
     cudaFree(c->d_rope_cs);
     cudaFree(c->d_q_rot);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < kMetaRing; ++i) {
         if (c->h_stage[i]) cudaFreeHost(c->h_stage[i]);
-        if (c->stage_done[i]) cudaEventDestroy(c->stage_done[i]);
+        if (c->copy_done[i]) cudaEventDestroy(c->copy_done[i]);
+        if (c->batch_end[i]) cudaEventDestroy(c->batch_end[i]);
     }
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     for (auto& t : c->ring) {
         if (t.start) cudaEventDestroy(t.start);
         if (t.stop) cudaEventDestroy(t.stop);
@@ -235,6 +239,9 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     float f_pf_tokens = 0, f_dec = 0, f_sum_ctx = 0, f_max_ctx = 0, f_pf_proc = 0, f_pf_proc_max = 0;
     int32_t n_prefill = 0, n_decode = 0;
     double alg_pairs = 0, alg_keys = 0;
+#ifdef CP_DEBUG_VARIANTS
+    const uint32_t epoch = ++c->mark_epoch;
+#endif
     for (int j = 0; j < n_reqs; ++j) {
         const cp_req_desc& r = reqs[j];
         if (r.q_len < 1 || r.ctx_off < 0 || r.n_blocks < 0 || (!r.block_table && r.n_blocks > 0)) {
@@ -250,14 +257,22 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
             return CP_EINVAL;
         }
         const int used_pages = (int)((kv_len + B - 1) / B);
-        for (int p = 0; p < used_pages; ++p)
+        for (int p = 0; p < used_pages; ++p) {
             if (r.block_table[p] < 0 || r.block_table[p] >= c->cfg.num_blocks) {
                 cp_set_error("cp_build_batch: request %d: page id %d out of range", j, r.block_table[p]);
                 return CP_EINVAL;
             }
+#ifdef CP_DEBUG_VARIANTS
+            if (c->page_mark[r.block_table[p]] == epoch) {
+                cp_set_error("cp_build_batch: request %d: page id %d appears twice in the batch", j, r.block_table[p]);
+                return CP_EINVAL;
+            }
+            c->page_mark[r.block_table[p]] = epoch;
+#endif
+        }
         T += r.q_len;
         P += used_pages;
-        if (r.q_len == 1) {
+        if (r.q_len == 1 && !(r.flags & CP_REQ_PREFILL)) {
             ++n_decode; f_dec += 1; f_sum_ctx += (float)(r.ctx_off + 1);
             f_max_ctx = std::max(f_max_ctx, (float)(r.ctx_off + 1));
         } else {
@@ -283,9 +298,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     // Measured on B200: P = 12 for both kinds cost 14 % on the chunks of
     // configs[2] and 20 % on configs[1].
     int per_sm[2] = {1, 2};
-    if (!c->use_dl) per_sm[0] = per_sm[1] = 12;
-    if (const char* e = getenv("CP_X_PT")) per_sm[0] = atoi(e);                   // experiments only
-    if (const char* e = getenv("CP_X_PS")) per_sm[1] = atoi(e);
+    if (!c->use_tc) per_sm[0] = per_sm[1] = 12;                   // SIMT cross-check kernel (debug builds): one CTA per item
     int chunk_of[2];
     for (int k = 0; k < 2; ++k) {
         const int64_t total = total_tiles[0] + total_tiles[1];     // the lanes share the SMs: mean load of the whole batch
@@ -363,7 +376,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     // their emission order (the L2-sharing neighbourhoods above)
     auto cost_of = [](const WorkItem& w) { return (w.kv_end - w.kv_begin + 4 * kKeyTile - 1) / (4 * kKeyTile); };
     for (const WorkItem& w : c->items) { max_cost = std::max(max_cost, cost_of(w)); n_tile_items += w.kind == kKindTile; }
-    const size_t kind_stride = c->use_dl ? (size_t)max_cost + 1 : 0;
+    const size_t kind_stride = c->use_tc ? (size_t)max_cost + 1 : 0;
     auto bucket_of = [&](const WorkItem& w) { return (w.kind == kKindSwap ? kind_stride : 0) + (size_t)(max_cost - cost_of(w)); };
     c->bucket.assign(kind_stride + (size_t)max_cost + 2, 0);
     for (const WorkItem& w : c->items) ++c->bucket[bucket_of(w) + 1];
@@ -372,8 +385,12 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     for (const WorkItem& w : c->items) c->sorted[c->bucket[bucket_of(w)]++] = w;
 
     // ---- pack into pinned staging ------------------------------------------------------------
-    const int si = c->stage_idx ^ 1;
-    if (c->stage_used[si]) CP_CUDA(cudaEventSynchronize(c->stage_done[si]));   // long since done
+    // the batch that ends here: every step it will ever run has been enqueued on step_stream by now
+    if (c->slot >= 0) CP_CUDA(cudaEventRecord(c->batch_end[c->slot], c->step_stream));
+    const int si = (c->slot + 1) % kMetaRing;
+    // staging slot si was last used kMetaRing batches ago: its copy finished long since; the host waits here
+    // only when it runs more than kMetaRing - 1 batches ahead of the device (include/cp.h)
+    if (c->slot_used[si]) CP_CUDA(cudaEventSynchronize(c->copy_done[si]));
     uint8_t* h = c->h_stage[si];
     size_t off = 0;
     auto place = [&](size_t bytes) { size_t o = off; off += align_up(bytes, 16); return o; };
@@ -412,20 +429,26 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     }
     std::memcpy(h + o_cb, c->combines.data(), sizeof(CombineItem) * c->combines.size());
 
-    if (off > 0) CP_CUDA(cudaMemcpyAsync(c->d_meta, h, off, cudaMemcpyHostToDevice, stream));
-    CP_CUDA(cudaEventRecord(c->stage_done[si], stream));
-    c->stage_used[si] = true;
-    c->stage_idx = si;
+    // the copy runs on the library's own stream, next to the previous batch's steps; it waits only for the
+    // steps that read this device slot kMetaRing batches ago, and the caller's stream waits for the copy
+    uint8_t* d_meta = c->d_meta[si];
+    if (c->slot_used[si]) CP_CUDA(cudaStreamWaitEvent(c->copy_stream, c->batch_end[si], 0));
+    if (off > 0) CP_CUDA(cudaMemcpyAsync(d_meta, h, off, cudaMemcpyHostToDevice, c->copy_stream));
+    CP_CUDA(cudaEventRecord(c->copy_done[si], c->copy_stream));
+    CP_CUDA(cudaStreamWaitEvent(stream, c->copy_done[si], 0));
+    c->slot_used[si] = true;
+    c->slot = si;
+    c->step_stream = stream;
 
     BatchMeta& m = c->meta;
-    m.cu_q = reinterpret_cast<const int32_t*>(c->d_meta + o_cu);
-    m.q_len = reinterpret_cast<const int32_t*>(c->d_meta + o_ql);
-    m.ctx_off = reinterpret_cast<const int32_t*>(c->d_meta + o_co);
-    m.bt_off = reinterpret_cast<const int32_t*>(c->d_meta + o_bo);
-    m.block_table = reinterpret_cast<const int32_t*>(c->d_meta + o_bt);
-    m.tok_req = reinterpret_cast<const int32_t*>(c->d_meta + o_tr);
-    m.work = reinterpret_cast<const WorkItem*>(c->d_meta + o_wk);
-    m.combine = reinterpret_cast<const CombineItem*>(c->d_meta + o_cb);
+    m.cu_q = reinterpret_cast<const int32_t*>(d_meta + o_cu);
+    m.q_len = reinterpret_cast<const int32_t*>(d_meta + o_ql);
+    m.ctx_off = reinterpret_cast<const int32_t*>(d_meta + o_co);
+    m.bt_off = reinterpret_cast<const int32_t*>(d_meta + o_bo);
+    m.block_table = reinterpret_cast<const int32_t*>(d_meta + o_bt);
+    m.tok_req = reinterpret_cast<const int32_t*>(d_meta + o_tr);
+    m.work = reinterpret_cast<const WorkItem*>(d_meta + o_wk);
+    m.combine = reinterpret_cast<const CombineItem*>(d_meta + o_cb);
     m.n_reqs = n_reqs;
     m.n_tokens = (int32_t)T;
     m.n_work = (int32_t)n_items;
@@ -489,6 +512,7 @@ extern "C" int cp_enable_rope(cp_ctx* c, const double* inv_freq) {
 // ------------------------------------------------------------------------------------
 // H2-H5: cp_attention_step
 // ------------------------------------------------------------------------------------
+#ifdef CP_DEBUG_VARIANTS
 template <int D>
 static int launch_simt(cp_ctx* c, const __nv_bfloat16* q, const __nv_bfloat16* cache,
                        __nv_bfloat16* out, cudaStream_t stream) {
@@ -503,8 +527,8 @@ static int launch_simt(cp_ctx* c, const __nv_bfloat16* q, const __nv_bfloat16* c
     }
     return CP_OK;
 }
+#endif
 
-#ifdef CP_WITH_TC
 typedef CUresult (*cuTensorMapEncodeTiled_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                              const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
                                              CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
@@ -529,7 +553,7 @@ static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out) {
     //   d2 D/64 halves of a row (stride 128 B)     d3 2 row groups (stride 8*D*2)
     //   d4 slab index (stride 16*D*2)
     // The box lands in smem as [row group][half][8 rows][128 B]: 8-row groups of each half are
-    // D/64 KiB apart for the whole 128-key tile, which is a legal UMMA SBO (see cp_kernels_tc.cuh).
+    // D/64 KiB apart for the whole 128-key tile, which is a legal UMMA SBO (see cp_kernels_dl.cuh).
     const cuuint64_t rowb = (cuuint64_t)sh.D * 2;
     const cuuint64_t dims[5] = {64, 8, (cuuint64_t)sh.D / 64, 2, (cuuint64_t)c->cfg.num_blocks * 2 * sh.Hkv};
     const cuuint64_t strides[4] = {rowb, 128, 8 * rowb, 16 * rowb};
@@ -553,22 +577,16 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
     int rc = get_tmap(c, kv_cache, &tmap);
     if (rc != CP_OK) return rc;
     if (!c->tc_attr_set) {
-        CP_CUDA(cudaFuncSetAttribute(attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcLayout<D>::kTotal));
         CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D>::kTotal));
         CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D>::kTotal));
         c->tc_attr_set = true;
     }
     if (m.n_work > 0) {
         const int grid = std::min(c->n_sm, m.n_work);
-        if (c->use_dl) {
-            dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
-            // tensor-bound batches take the instantiation that moves a quarter of the exponentials to the FMA pipe
-            CP_CUDA(launch_pdl(c->tensor_bound ? dl::attn_dl_kernel<D, true> : dl::attn_dl_kernel<D, false>, dim3(grid),
-                               dim3(dl::kThreads), dl::Layout<D>::kTotal, stream, p, *tmap));
-        } else {
-            TcParams p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, c->d_prof};
-            attn_tc_kernel<D><<<grid, kTcThreads, TcLayout<D>::kTotal, stream>>>(p, *tmap);
-        }
+        dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter};
+        // tensor-bound batches take the instantiation that moves a quarter of the exponentials to the FMA pipe
+        CP_CUDA(launch_pdl(c->tensor_bound ? dl::attn_dl_kernel<D, true> : dl::attn_dl_kernel<D, false>, dim3(grid),
+                           dim3(dl::kThreads), dl::Layout<D>::kTotal, stream, p, *tmap));
         CP_CUDA(cudaGetLastError());
         ++*launches;
         c->info.grid_attn = grid;
@@ -587,7 +605,6 @@ static int launch_tc(cp_ctx* c, const __nv_bfloat16* q, __nv_bfloat16* kv_cache,
     return c->shape.D == 128 ? launch_tc_d<128>(c, q, kv_cache, out, stream, launches)
                              : launch_tc_d<64>(c, q, kv_cache, out, stream, launches);
 }
-#endif
 
 static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new, const void* v_new,
                           void* kv_cache, void* out, void* stream_, bool rope) {
@@ -611,6 +628,7 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
         return CP_EINVAL;
     }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    c->step_stream = stream;
     const BatchMeta& m = c->meta;
     TimedStep& ts = c->ring[(size_t)(c->ring_head % kRing)];
     CP_CUDA(cudaEventRecord(ts.start, stream));
@@ -638,13 +656,8 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
             ++launches;
         }
         int rc;
-#ifdef CP_WITH_TC
-        if (c->use_tc) {
-            rc = launch_tc(c, static_cast<const __nv_bfloat16*>(q), static_cast<__nv_bfloat16*>(kv_cache),
-                           static_cast<__nv_bfloat16*>(out), stream, &launches);
-        } else
-#endif
-        {
+#ifdef CP_DEBUG_VARIANTS
+        if (!c->use_tc) {
             rc = c->shape.D == 128
                      ? launch_simt<128>(c, static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(kv_cache),
                                         static_cast<__nv_bfloat16*>(out), stream)
@@ -653,6 +666,11 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
             launches += (m.n_work > 0) + (m.n_combine > 0);
             c->info.grid_attn = m.n_work;
             c->info.grid_combine = m.n_combine;
+        } else
+#endif
+        {
+            rc = launch_tc(c, static_cast<const __nv_bfloat16*>(q), static_cast<__nv_bfloat16*>(kv_cache),
+                           static_cast<__nv_bfloat16*>(out), stream, &launches);
         }
         if (rc != CP_OK) return rc;
     }
@@ -705,15 +723,6 @@ extern "C" int cp_set_memory_stats(cp_ctx* c, float used, float freemb, float al
     c->mem_stats[0] = used; c->mem_stats[1] = freemb; c->mem_stats[2] = allocated; c->mem_stats[3] = reserved;
     return CP_OK;
 }
-
-#if defined(CP_TC_PROF) || defined(CP_TC_PROF2) || defined(CP_TL)
-// debug builds only (not part of include/cp.h): per-CTA wait-time profile of the last launch
-extern "C" int cp_debug_prof(cp_ctx* c, unsigned long long* host_buf, int n_ctas) {
-    if (!c->d_prof) return CP_ESTATE;
-    cudaDeviceSynchronize();
-    return cudaMemcpy(host_buf, c->d_prof, sizeof(unsigned long long) * 32 * n_ctas, cudaMemcpyDeviceToHost) == cudaSuccess ? CP_OK : CP_ECUDA;
-}
-#endif
 
 extern "C" int cp_get_batch_info(cp_ctx* c, cp_batch_info* info) {
     if (!c || !info) return CP_EINVAL;

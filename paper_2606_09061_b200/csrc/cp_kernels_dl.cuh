@@ -78,24 +78,6 @@ struct Layout {
     static constexpr uint32_t kTotal = kOffMisc + kMiscBytes + 1024;   // + slack to align the base to 1024
 };
 
-// Optional role-level wait-time profile of lane T (build with -DCP_TC_PROF; debugging aid only).
-#ifdef CP_TC_PROF
-#define DL_T0 long long t0__ = clock64()
-#define DL_ACC(id) do { const long long t1__ = clock64(); if ((threadIdx.x & 31) == 0) atomicAdd(&ls->prof[id], (unsigned long long)(t1__ - t0__)); t0__ = t1__; } while (0)
-#else
-#define DL_T0 do {} while (0)
-#define DL_ACC(id) do {} while (0)
-#endif
-
-// Optional event timeline of CTA 0, lane T (build with -DCP_TL; debugging aid only): records
-// (event id, half-tile counter, clock) triples into p.prof.
-#ifdef CP_TL
-// cheap recording: 32-bit clock into lane T's small region (idle during tile items) of CTA 0, slot [half-tile][event];
-// copied out at the end.  190 half-tiles fit.
-#define DL_TL(ev, idx) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (idx) < 190u) { unsigned c__; asm volatile("mov.u32 %0, %%clock;" : "=r"(c__)); reinterpret_cast<volatile unsigned*>(reinterpret_cast<uint8_t*>(ls) - Layout<D>::kOffMisc + (kStagesT + kStagesS) * Layout<D>::kSlotBytes)[(idx) * 16 + (ev)] = c__; } } while (0)
-#else
-#define DL_TL(ev, idx) do {} while (0)
-#endif
 
 struct LaneState {              // one per lane, in the misc region
     uint64_t kv_full[kMaxStages];
@@ -117,9 +99,6 @@ struct LaneState {              // one per lane, in the misc region
     WorkItem items[kItemRing];  // published by the lane's producer; kind < 0 = no more work
     float cmax[2][4][16];       // swap kind: per-warp column maxima, double buffered
     float lsum[4][16];          // swap kind: per-warp column sums at the end of an item
-#ifdef CP_TC_PROF
-    unsigned long long prof[16];
-#endif
 };
 
 struct Misc {
@@ -136,7 +115,6 @@ struct Params {
     float* part_o;
     float2* part_ml;
     int32_t* counters;          // [0] next tile item, [1] next swap item, [2] finished CTAs
-    unsigned long long* prof;   // [grid][16] role wait-time profile (-DCP_TC_PROF builds), else unused
 };
 
 // element e of a half-tile row: MUFU or FMA-pipe exponential (e is a constant after unrolling)
@@ -256,24 +234,12 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             const int n_pages = min(8, n_pages_item - tile * 8);          // 1..8
             const uint32_t ld = ld_base + i;
             const uint32_t slot = ld % kStages;
-            { DL_T0; ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1); DL_ACC(8); }
+            ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1);
             const bool leader = ptx::elect_one();
-#if defined(DL_X_NOTMA) || defined(DL_X_S_NOTMA)
-#ifdef DL_X_S_NOTMA
-            const bool no_tma = LANE == 1;
-#else
-            const bool no_tma = true;
-#endif
-            if (leader) { if (no_tma) ptx::mbar_arrive(&ls->kv_full[slot]); else ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u); }
-            uint8_t* dst = kv_base + slot * L::kSlotBytes;
-#pragma unroll
-            for (int j = 0; j < (no_tma ? 0 : 8); ++j) {
-#else
             if (leader) ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u);
             uint8_t* dst = kv_base + slot * L::kSlotBytes;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-#endif
                 const int pg = __shfl_sync(0xffffffffu, cur, (tile & 3) * 8 + j);
                 if (j < n_pages) {
                     const int slab = (pg * 2 + is_v) * p.sh.Hkv + kv_head;
@@ -284,6 +250,24 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
         }
         ld_base += 2 * n_tiles;
     }
+}
+
+// Rows [first, 128) of the LAST V tile of an item are not keys of the request: slots of the last page
+// past kv_end hold whatever the pool held (another request's rows, NaN in a torch.empty pool), and
+// pages the tile does not have were never loaded (stale shared memory).  Masked P is exactly 0, but
+// 0 x NaN in the PV product is NaN, so the PV issuer zeroes those rows -- generic-proxy stores after
+// the TMA has landed, made visible to the tensor core's async proxy -- before it issues the block.
+// K needs nothing: a NaN score of a masked key is removed by select, never by arithmetic.
+template <int D>
+__device__ __forceinline__ void zero_v_tail(uint32_t v_tile, int first) {
+    using L = Layout<D>;
+    constexpr int kPerRow = L::kHalves * 8;                 // 16-byte chunks per key row
+    for (int i = first * kPerRow + (int)(threadIdx.x & 31); i < kKeyTile * kPerRow; i += 32) {
+        const int r = i / kPerRow, c = i % kPerRow;
+        ptx::st_shared_zero16(v_tile + (r >> 3) * L::kGroupBytes + (c >> 3) * 1024 + (r & 7) * 128 + (c & 7) * 16);
+    }
+    ptx::fence_proxy_async_smem();
+    __syncwarp();
 }
 
 // ------------------------------------------------------------------------------------------
@@ -315,9 +299,7 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
     const uint32_t idesc_pv = ptx::umma_idesc_bf16(128, D, false, true);
     const uint32_t gh0 = gh;
     if (ROLE == 1) {
-        DL_T0;
         ptx::mbar_wait(&ls->q_full[0], ic[0] & 1);
-        DL_ACC(7);
         ptx::tc_fence_after();
     }
     ++ic[0];
@@ -329,12 +311,8 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
             // load order of the producers: K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1)
             const uint32_t ld = ld_base + (t == 0 ? 0 : 2 * t - 1);
             const uint32_t slot = ld % kStages;
-            DL_T0;
             if (j >= 4) ptx::mbar_wait(&ls->pv_issued[buf], ((g - 4) >> 2) & 1);      // PV(j-4) (same S buffer) is in the pipe
-            DL_TL(1, g);
             if (h == 0) ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
-            DL_TL(2, g);
-            DL_ACC(4);
             ptx::tc_fence_after();
             const uint32_t k_half = kv_base + slot * L::kSlotBytes + h * 8 * L::kGroupBytes;   // rows 64 h .. 64 h + 63
             const uint32_t d_tmem = tmem + buf * 64;
@@ -349,18 +327,14 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
                 ptx::umma_commit(&ls->ts_full[buf]);
             }
             __syncwarp();
-            DL_TL(3, g);
-            DL_ACC(11);
         } else {
             const uint32_t ld = ld_base + (t == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * t + 2);
             const uint32_t slot = ld % kStages;
-            DL_T0;
             ptx::mbar_wait(&ls->tp_full[buf], (g >> 2) & 1);
-            DL_TL(4, g);
-            DL_ACC(5);
-            if (h == 0) ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
-            DL_TL(5, g);
-            DL_ACC(6);
+            if (h == 0) {
+                ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+                if (t == n_tiles - 1 && (n_keys & (kKeyTile - 1))) zero_v_tail<D>(kv_base + slot * L::kSlotBytes, n_keys & (kKeyTile - 1));
+            }
             ptx::tc_fence_after();
             const uint32_t v_half = kv_base + slot * L::kSlotBytes + h * 4 * L::kPageBytes;     // keys 64 h .. 64 h + 63
             const uint32_t d_tmem = tmem + col_o(0);
@@ -377,8 +351,6 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
                 ptx::mbar_arrive(&ls->pv_issued[buf]);
             }
             __syncwarp();
-            DL_TL(6, g);
-            DL_ACC(12);
         }
     }
     gh += nh;
@@ -390,7 +362,8 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
                                          uint32_t& ld_base, uint32_t& gt, uint32_t& gp, uint32_t (&ic)[2], uint32_t& gpt) {
     using L = Layout<D>;
     constexpr int kStages = LANE == 0 ? kStagesT : kStagesS;
-    const int n_tiles = (__shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0) + kKeyTile - 1) / kKeyTile;
+    const int n_keys = __shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0);
+    const int n_tiles = (n_keys + kKeyTile - 1) / kKeyTile;
     const bool swap = LANE == 1 || __shfl_sync(0xffffffffu, it.kind, 0) == kKindSwap;
     const bool all = ROLE == 0 || swap;        // this warp issues both kinds of block
     if (!swap) {
@@ -413,9 +386,7 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
     const uint32_t g0 = gt, t0 = gpt;          // global tile counter / tile-kind tile counter at item start
 
     if (do_qk) {
-        DL_T0;
         ptx::mbar_wait(&ls->q_full[set], ic[set] & 1);
-        DL_ACC(7);
         ptx::tc_fence_after();
     }
     ++ic[set];
@@ -424,10 +395,8 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
     auto issue_qk = [&](int t) {
         const uint32_t ld = ld_base + (t == 0 ? 0 : 2 * t - 1);
         const uint32_t slot = ld % kStages, buf = (g0 + t) & 1;
-        DL_T0;
         if (!all && t >= 2) ptx::mbar_wait(&ls->pv_issued[(t0 + t) & 1], ((t0 + t - 2) >> 1) & 1);   // PV(t-2) is in the pipe
         ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
-        DL_ACC(4);
         ptx::tc_fence_after();
         const uint32_t k_tile = kv_base + slot * L::kSlotBytes;
         const uint32_t d_tmem = tmem + col_s(LANE, buf);
@@ -435,11 +404,7 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
             const uint64_t k_desc0 = ptx::umma_desc_sw128(k_tile, 16, L::kGroupBytes);
             const uint64_t q_desc0 = ptx::umma_desc_sw128(small, 16, 1024);
 #pragma unroll
-#ifdef DL_X_S_NOMMA
-            for (int ks = 0; ks < (swap ? 0 : D / 16); ++ks) {
-#else
             for (int ks = 0; ks < D / 16; ++ks) {
-#endif
                 const uint32_t koff = (ks >> 2) * 1024 + (ks & 3) * 32;                // K slot: halves 1 KB apart
                 const uint64_t k_desc = ptx::umma_desc_advance(k_desc0, koff);
                 if (LANE == 0 && !swap) {
@@ -453,29 +418,22 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
             ptx::umma_commit(&ls->s_full[buf]);
         }
         __syncwarp();
-        DL_ACC(11);
     };
     auto issue_pv = [&](int t) {
         const uint32_t ld = ld_base + (t == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * t + 2);
         const uint32_t slot = ld % kStages, buf = (g0 + t) & 1;
-        DL_T0;
         ptx::mbar_wait(&ls->p_full[set][gp & 1], (gp >> 1) & 1);
-        DL_ACC(5);
         ++gp;
         ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
-        DL_ACC(6);
-        ptx::tc_fence_after();
         const uint32_t v_tile = kv_base + slot * L::kSlotBytes;
+        if (t == n_tiles - 1 && (n_keys & (kKeyTile - 1))) zero_v_tail<D>(v_tile, n_keys & (kKeyTile - 1));
+        ptx::tc_fence_after();
         const uint32_t d_tmem = tmem + col_o(LANE);
         if (ptx::elect_one()) {
             const uint64_t v_desc0 = ptx::umma_desc_sw128(v_tile, 1024, L::kGroupBytes);
             const uint64_t p_desc0 = ptx::umma_desc_sw128(small + 4096 + buf * 4096, 16, 1024);      // P^T is double buffered
 #pragma unroll
-#ifdef DL_X_S_NOMMA
-            for (int ks = 0; ks < (swap ? 0 : kKeyTile / 16); ++ks) {
-#else
             for (int ks = 0; ks < kKeyTile / 16; ++ks) {
-#endif
                 // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO)
                 const uint64_t v_desc = ptx::umma_desc_advance(v_desc0, ks * L::kPageBytes);
                 if (LANE == 0 && !swap) {
@@ -490,7 +448,6 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
             if (!all) ptx::mbar_arrive(&ls->pv_issued[(t0 + t) & 1]);
         }
         __syncwarp();
-        DL_ACC(12);
     };
 
     // QK(t+1) is issued before PV(t) so the softmax of tile t overlaps the next score MMA.  p_full is
@@ -546,7 +503,6 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
     const float scale = sh.sm_scale * 1.4426950408889634f;
     const uint32_t t_row = tmem + (lane_base << 16);
 
-    DL_T0;
     // ---- Q row -> TMEM (A operand of QK^T): column j holds elements (2j, 2j+1)
     {
         const uint4* src = reinterpret_cast<const uint4*>(p.q + ((int64_t)tok * sh.Hq + head) * D);
@@ -564,7 +520,6 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         ptx::tc_fence_before();
         warp_arrive(&ls->q_full[0]);
     }
-    DL_ACC(9);
 
     const int limit = valid_row ? min(it.kv_end, ctx + it.q_start + (row >> gs) + 1) : 0;   // causal, diagonal inclusive
     float m_ref = -INFINITY, l = 0.f;
@@ -575,24 +530,11 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         const uint32_t buf = gh & 3;
         const uint32_t t_s = t_row + buf * 64;
         ptx::mbar_wait(&ls->ts_full[buf], (gh >> 2) & 1);
-        if (lane_base == 0) DL_TL(7, gh);
-        DL_ACC(0);
         ptx::tc_fence_after();
-#ifdef DL_X_NOTMEM
-        { l += 1.f; ptx::tc_fence_before(); warp_arrive(&ls->tp_full[buf]); ++gh; continue; }
-#endif
         uint32_t sr[64];
         ptx::tmem_ld32(t_s, sr);
         ptx::tmem_ld32(t_s + 32, sr + 32);
         ptx::tmem_wait_ld();
-        if (lane_base == 0) DL_TL(8, gh);
-#ifdef DL_X_NOSOFTMAX
-        { uint32_t pk[32];
-#pragma unroll
-          for (int i = 0; i < 32; ++i) pk[i] = 0x3c003c00u ^ (sr[i] & 1u);
-          ptx::tmem_st32(t_s, pk);
-          l += 1.f; ptx::tmem_wait_st(); ptx::tc_fence_before(); warp_arrive(&ls->tp_full[buf]); ++gh; continue; }
-#endif
         const int nvalid = max(0, min(64, limit - ts));
         float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};      // independent max chains
         if (nvalid == 64) {
@@ -611,7 +553,6 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
             rescale = true;
         }
         const float neg_m = (m_ref == -INFINITY) ? 0.f : -m_ref;
-        if (lane_base == 0) DL_TL(9, gh);
         float sm[4] = {0.f, 0.f, 0.f, 0.f};             // independent sum chains
         uint32_t pk[32];                                // 64 scores -> 32 packed P columns
         if (nvalid == 64) {
@@ -631,9 +572,7 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
                 pk[i >> 1] = pack_bf16(a, b);
             }
         }
-        if (lane_base == 0) DL_TL(10, gh);
         ptx::tmem_st32(t_s, pk);
-        if (lane_base == 0) DL_TL(11, gh);
         l = l * alpha + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
         if (j > 0 && __any_sync(0xffffffffu, rescale)) {
             ptx::mbar_wait(&ls->tpv_done[(gh - 1) & 3], ((gh - 1) >> 2) & 1);      // PV(j-1) (and all before) done: O readable
@@ -651,14 +590,11 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         ptx::tmem_wait_st();
         ptx::tc_fence_before();
         warp_arrive(&ls->tp_full[buf]);
-        if (lane_base == 0) DL_TL(12, gh);
-        DL_ACC(1);
         ++gh;
     }
 
     // ---- epilogue: O row from TMEM (one load batch) -> out (bf16, normalised) or split workspace (fp32, unnormalised)
     ptx::mbar_wait(&ls->tpv_done[(gh - 1) & 3], ((gh - 1) >> 2) & 1);
-    DL_ACC(2);
     ptx::tc_fence_after();
     const float inv = 1.f / l;
     uint32_t o[D];
@@ -682,7 +618,6 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         }
     }
     ptx::tc_fence_before();
-    DL_ACC(3);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -785,9 +720,7 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
             ptx::tmem_st<RC>(t_row + col_o(LANE), o);
             ptx::tmem_wait_st();
         }
-#ifndef DL_X_S_NOFENCE
         ptx::fence_proxy_async_smem();
-#endif
         ptx::tc_fence_before();
         warp_arrive(&ls->p_full[1][gp & 1]);
         ++gt;
@@ -840,7 +773,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
     uint32_t gt = 0, item_cnt = 0, gh_tile = 0, gp_swap = 0;      // gt / gp_swap: swap-kind tiles; gh_tile: tile-kind half-tiles
     for (;;) {
         const uint32_t islot = item_cnt % kItemRing;
-        { DL_T0; ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1); DL_ACC(10); }
+        ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1);
         const WorkItem it = ls->items[islot];
         warp_arrive(&ls->item_empty[islot]);
         if (it.kind < 0) break;
@@ -895,15 +828,8 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         ptx::prefetch_tmap(&tmap);
     }
     if (warp == 6) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
-#ifdef CP_TC_PROF
-    if (threadIdx.x < 32) misc->lane[threadIdx.x >> 4].prof[threadIdx.x & 15] = 0;
-    const long long t_start__ = clock64();
-#endif
-    // stale shared memory may hold NaN bit patterns; tiles are only partly overwritten by short
-    // requests, and 0 x NaN would poison the accumulators
-    for (uint32_t i = threadIdx.x * 16; i < L::kOffMisc; i += kThreads * 16)
-        *reinterpret_cast<uint4*>(smem + i) = make_uint4(0, 0, 0, 0);
-    ptx::fence_proxy_async_smem();
+    // shared memory is NOT cleared: nothing stale in it can reach a result (masked scores are removed by
+    // select, the rows of a V tile past the item's last key are zeroed by the PV issuer, zero_v_tail)
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
@@ -929,14 +855,6 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 6) ptx::tmem_dealloc(misc->tmem_base, kTmemCols);
-#ifdef CP_TL
-    if (blockIdx.x == 0 && p.prof) for (uint32_t i = threadIdx.x; i < 190 * 16; i += kThreads) p.prof[i] = reinterpret_cast<const unsigned*>(smem + (kStagesT + kStagesS) * L::kSlotBytes)[i];
-#endif
-#ifdef CP_TC_PROF
-    if (threadIdx.x == 0) { misc->lane[0].prof[15] = (unsigned long long)(clock64() - t_start__); misc->lane[0].prof[13] -= (unsigned long long)t_start__; }
-    __syncthreads();
-    if (threadIdx.x < 32 && p.prof) p.prof[blockIdx.x * 32 + threadIdx.x] = misc->lane[threadIdx.x >> 4].prof[threadIdx.x & 15];
-#endif
     if (threadIdx.x == 0) {
         __threadfence();
         if (atomicAdd(&p.counters[2], 1) == (int)gridDim.x - 1) {      // last CTA re-arms the counters

@@ -1,8 +1,7 @@
 // cp_kernels_simt.cuh -- plain-ALU kernels of libcp for sm_100a:
 //   kv_append_kernel   H2: scatter the iteration's new K/V rows into their pages
-//   attn_simt_kernel   H3/H4 reference path: one warp per (token, q head) row, online
-//                      softmax in fp32, no tensor cores (kernel_variant = 1; also the
-//                      bisecting aid next to the tcgen05 path)
+//   attn_simt_kernel   H3/H4 cross-check for bisecting (-DCP_DEBUG_VARIANTS builds only,
+//                      kernel_variant = 1): one warp per (token, q head) row, no tensor cores
 //   combine_kernel     H5: LSE merge of split-KV partials -> bf16 out
 // Operation defined in include/cp.h / DESIGN.md section 2.
 #pragma once
@@ -135,8 +134,9 @@ __global__ void kv_append_rope_kernel(BatchMeta meta, Shape sh, const uint4* __r
     }
 }
 
+#ifdef CP_DEBUG_VARIANTS
 // ---------------------------------------------------------------------------------
-// Reference attention: CTA per work item, warp per row, lane owns D/32 dims.
+// Cross-check attention (debug builds only, kernel_variant 1): CTA per work item, warp per row, lane owns D/32 dims.
 // Scores are kept in log2 units (q pre-scaled by sm_scale * log2 e).
 // ---------------------------------------------------------------------------------
 template <int D>
@@ -216,6 +216,8 @@ attn_simt_kernel(BatchMeta meta, Shape sh, const __nv_bfloat16* __restrict__ q,
         }
     }
 }
+
+#endif  // CP_DEBUG_VARIANTS
 
 // ---------------------------------------------------------------------------------
 // H5: out = sum_s w_s O_s / sum_s w_s l_s, w_s = 2^(m_s - max m).  One warp per (token, head) row

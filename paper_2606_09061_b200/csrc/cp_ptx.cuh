@@ -88,9 +88,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 #else
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-#ifdef DL_X_NANOSLEEP
-        __nanosleep(DL_X_NANOSLEEP);
-#endif
         if (++spins > kWaitSpinLimit) __trap();
     }
 #endif
@@ -99,6 +96,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // ---- proxies / fences ---------------------------------------------------------------------
 __device__ __forceinline__ void fence_proxy_async_smem() {      // generic-proxy smem writes -> async proxy
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void st_shared_zero16(uint32_t addr) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0u) : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -253,13 +253,9 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {
 }
 
 __device__ __forceinline__ float ex2(float x) {
-#ifdef DL_X_NOEXP
-    return x * 0.001f;          // timing experiment only
-#else
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
-#endif
 }
 // 2^x on the FMA pipe (Cody-Waite split + degree-3 near-minimax polynomial on [-0.5, 0.5], max
 // relative error 7.5e-5, far below the bf16 rounding of P): MUFU.EX2 runs at 16 per clock per SM,

@@ -226,9 +226,19 @@ extern "C" {
 
 int cp_sched_create(const cp_sched_config* cfg, cp_sched** out) {
     if (!cfg || !out) { cp_set_error("cp_sched_create: null argument"); return CP_EINVAL; }
-    if (cfg->B_max < 1 || cfg->S_max < 0 || cfg->block_size < 1 || cfg->num_blocks < 1 ||
+    if (cfg->B_max < 1 || cfg->S_max < 1 || cfg->block_size < 1 || cfg->num_blocks < 1 ||
         cfg->Delta < 1 || cfg->L_min < 1 || cfg->num_blocks > INT32_MAX) {
         cp_set_error("cp_sched_create: bad limits");
+        return CP_EINVAL;
+    }
+    // Eq. 12 with C_max < 1 or L_min > B_max gives C_t = 0 on an empty batch: literal Eq. 14 then blocks every
+    // candidate for ever (no round could start a prefill) -- a configuration error, not a schedule
+    if (cfg->apc && (cfg->C_max < 1 || cfg->L_min > cfg->B_max)) {
+        cp_set_error("cp_sched_create: APC needs C_max >= 1 and L_min <= B_max");
+        return CP_EINVAL;
+    }
+    if (cfg->mode == CP_MODE_LPRS && !(cfg->lambda_u >= 0.0 && cfg->lambda_o >= 0.0)) {
+        cp_set_error("cp_sched_create: lambda_u, lambda_o must be >= 0 (Eq. 10; the paper takes lambda_o > lambda_u)");
         return CP_EINVAL;
     }
     size_t need = 16;
@@ -388,12 +398,12 @@ int cp_sched_next(cp_sched* s, int64_t now_us, cp_req_desc* out, int32_t cap, in
     for (int32_t slot : dec) {
         const Request& r = s->reqs[slot];
         out[k++] = cp_req_desc{r.req_id, 1, r.prompt_len + r.generated - 1, r.pages.data(),
-                               static_cast<int32_t>(r.pages.size())};
+                               static_cast<int32_t>(r.pages.size()), 0};
     }
     for (auto& pc : chosen) {
         const Request& r = s->reqs[pc.first];
         out[k++] = cp_req_desc{r.req_id, pc.second, r.prompt_len - r.remaining, r.pages.data(),
-                               static_cast<int32_t>(r.pages.size())};
+                               static_cast<int32_t>(r.pages.size()), CP_REQ_PREFILL};
     }
     *n_out = static_cast<int32_t>(n);
     s->pending = n > 0;

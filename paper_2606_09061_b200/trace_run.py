@@ -116,7 +116,11 @@ def run_trace(trace, *, Hq=32, Hkv=8, D=128, B=16, layers=32, pages_per_layer=20
         n = sched.cp_sched_next(now)
         digest.update(pack_batch(sched.descs, n))
         if n == 0:
-            now = sched.cp_sched_next_arrival()
+            nxt = sched.cp_sched_next_arrival()
+            if nxt < 0:
+                raise RuntimeError("scheduler has work but nothing is runnable and nothing will arrive "
+                                   "(a request that can never be admitted under this configuration)")
+            now = max(now, nxt)
             continue
         ctx.cp_build_batch(descs=sched.descs, n=n)
         if layer_gemms:

@@ -37,3 +37,23 @@ def test_dual_lane_kernel_sass_size_within_budget():
     # a runtime integer division shows up as a reciprocal sequence starting with I2F.U32.RP
     for body in sass.split("attn_dl_kernelILi128E")[1:]:
         assert body.split("Function :", 1)[0].count("I2F.U32.RP") <= 4, "runtime integer divisions crept back"
+
+
+@pytest.mark.skipif(shutil.which("cuobjdump") is None, reason="cuobjdump not on PATH")
+def test_attention_kernel_is_blackwell_native():
+    """The SASS of every attention-kernel instantiation holds tcgen05 MMAs (UTCHMMA), TMEM loads / stores
+    (LDTM / STTM) and TMA loads (UTMALDG), and no legacy tensor path (HMMA = mma.sync / wmma).  Counts are
+    committed under profiles/ (r02_sass_mnemonics.md)."""
+    lib = build.build()
+    sass = subprocess.run(["cuobjdump", "-sass", lib], check=True, capture_output=True, text=True).stdout
+    bodies = {}
+    for part in sass.split("Function : ")[1:]:
+        name, body = part.split("\n", 1)
+        bodies[name.strip()] = body
+    kernels = {k: v for k, v in bodies.items() if "attn_dl_kernel" in k}
+    assert len(kernels) >= 4
+    for name, body in kernels.items():
+        for mnemonic in ("UTCHMMA", "LDTM", "STTM", "UTMALDG", "UTCBAR"):
+            assert body.count(mnemonic) > 0, f"{name}: no {mnemonic} in the SASS"
+        assert not re.search(r"\bHMMA\b", body), f"{name}: legacy mma.sync path present"
+    assert not any("attn_simt" in k or "attn_tc" in k for k in bodies), "debug-only kernels in the shipped library"
