@@ -22,7 +22,9 @@
  * where K_j[t], V_j[t] live in page block_table_j[t / B], slot t % B.  A decode is
  * simply q_len == 1.  Stale data in page tails / other pages never influences the
  * result, whatever its bit pattern (NaN and Inf included): masked scores are removed by
- * select and the slots past a request's last key never reach the PV product.
+ * select, and every step first ZEROES the slots of each request's last page that lie past
+ * its last key (they belong to the request, hold no key, and later appends overwrite
+ * them), so that masked P = 0 never meets a NaN in the tensor-core PV product.
  */
 #ifndef CP_H_
 #define CP_H_
@@ -131,7 +133,8 @@ int cp_build_batch(cp_ctx* ctx, const cp_req_desc* reqs, int32_t n_reqs,
  *   k_new    DEVICE [T, Hkv, D] bf16, or NULL = caller already wrote the pages
  *   v_new    DEVICE [T, Hkv, D] bf16 (NULL iff k_new is NULL)
  *   kv_cache DEVICE the layer's pool [num_blocks][2][Hkv][B][D] bf16; the new rows are
- *            appended in place before anything attends (H2)
+ *            appended in place before anything attends (H2); the unused slots of each
+ *            request's last page are zeroed (also when k_new is NULL); nothing else is written
  *   out      DEVICE [T, Hq, D]  bf16, every row written
  * All pointers 16-byte aligned.  Errors: CP_ESTATE (no batch built), CP_EINVAL, CP_ECUDA. */
 int cp_attention_step(cp_ctx* ctx, int32_t layer, const void* q, const void* k_new,
@@ -178,6 +181,8 @@ typedef struct {
     int64_t n_partial_rows;      /* workspace rows in use                          */
     int32_t kernels_per_step;    /* kernel launches one cp_attention_step issues   */
     int32_t grid_attn, grid_combine;
+    int32_t split;               /* 1: tensor-bound batch, runs the SPLIT instantiation of the kernel (both
+                                    softmax warpgroups on every chunk tile); 0: dual-lane instantiation */
 } cp_batch_info;
 int cp_get_batch_info(cp_ctx* ctx, cp_batch_info* info);
 

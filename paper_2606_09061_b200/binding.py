@@ -54,7 +54,7 @@ class cp_batch_info(C.Structure):
     _fields_ = [("n_reqs", C.c_int32), ("n_tokens", C.c_int32), ("n_work_items", C.c_int32),
                 ("n_combine_items", C.c_int32), ("n_tc_items", C.c_int32),
                 ("n_partial_rows", C.c_int64), ("kernels_per_step", C.c_int32),
-                ("grid_attn", C.c_int32), ("grid_combine", C.c_int32)]
+                ("grid_attn", C.c_int32), ("grid_combine", C.c_int32), ("split", C.c_int32)]
 
 
 class cp_sched_config(C.Structure):

@@ -231,7 +231,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     if (!c || (!reqs && n_reqs > 0) || n_reqs < 0) { cp_set_error("cp_build_batch: bad argument"); return CP_EINVAL; }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const Shape& sh = c->shape;
-    const int B = sh.B, G = sh.G, TQ = c->tq;
+    const int B = sh.B, G = sh.G;
     if (n_reqs > c->cfg.max_reqs) { cp_set_error("cp_build_batch: %d requests > max_reqs %d", n_reqs, c->cfg.max_reqs); return CP_ECAPACITY; }
 
     // ---- validate + totals ------------------------------------------------------------
@@ -279,6 +279,19 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
             ++n_prefill; f_pf_tokens += (float)r.q_len; f_pf_proc += (float)r.ctx_off;
             f_pf_proc_max = std::max(f_pf_proc_max, (float)r.ctx_off);
         }
+    }
+    // SURVEY.md 8(d) formulas: FLOPs = 4 D Hq pairs; bytes = KV once per request and KV head + Q + out.  A batch
+    // that is tensor-bound at the nominal B200 rates runs the SPLIT instantiation of the kernel: both softmax
+    // warpgroups of a CTA work on every chunk tile (cp_kernels_dl.cuh).
+    bool tensor_bound;
+    {
+        const double flops = 4.0 * sh.D * sh.Hq * alg_pairs;
+        const double bytes = 2.0 * alg_keys * sh.Hkv * sh.D * 2 + 2.0 * (double)T * sh.Hq * sh.D * 2;
+        tensor_bound = c->use_tc && flops / 2.25e15 > bytes / 8e12;
+    }
+    const int TQ = c->tq;                                // tokens per tile-kind item
+    for (int j = 0; j < n_reqs; ++j) {
+        const cp_req_desc& r = reqs[j];
         for (int q0 = 0; q0 < r.q_len; q0 += TQ) {
             const int qt = std::min(TQ, r.q_len - q0);
             const int64_t lim = (int64_t)r.ctx_off + q0 + qt;
@@ -458,16 +471,12 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     int32_t n_tc = 0;
     if (c->use_tc) n_tc = (int32_t)n_items;
     c->info = cp_batch_info{n_reqs, (int32_t)T, (int32_t)n_items, (int32_t)c->combines.size(), n_tc,
-                            partial_rows, 0, 0, 0};
+                            partial_rows, 0, 0, 0, tensor_bound ? 1 : 0};
     c->feat[0] = f_pf_tokens; c->feat[1] = f_dec; c->feat[2] = (float)n_reqs; c->feat[3] = f_sum_ctx;
     c->feat[4] = f_max_ctx; c->feat[5] = f_pf_proc; c->feat[6] = f_pf_proc_max;
     c->n_prefill = n_prefill;
     c->n_decode = n_decode;
-    {   // SURVEY.md 8(d) formulas: FLOPs = 4 D Hq pairs; bytes = KV once per request and KV head + Q + out
-        const double flops = 4.0 * sh.D * sh.Hq * alg_pairs;
-        const double bytes = 2.0 * alg_keys * sh.Hkv * sh.D * 2 + 2.0 * (double)T * sh.Hq * sh.D * 2;
-        c->tensor_bound = flops / 2.25e15 > bytes / 8e12;
-    }
+    c->tensor_bound = tensor_bound;
     c->have_batch = true;
     ++c->iter;
     if (c->d_rope_cs && T > 0) {       // positions changed: (cos, sin) table of this batch, same stream as the copy
@@ -577,16 +586,20 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
     int rc = get_tmap(c, kv_cache, &tmap);
     if (rc != CP_OK) return rc;
     if (!c->tc_attr_set) {
-        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D>::kTotal));
-        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D>::kTotal));
+        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D, false>::kTotal));
+        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D, true>::kTotal));
         c->tc_attr_set = true;
     }
     if (m.n_work > 0) {
         const int grid = std::min(c->n_sm, m.n_work);
         dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter};
-        // tensor-bound batches take the instantiation that moves a quarter of the exponentials to the FMA pipe
-        CP_CUDA(launch_pdl(c->tensor_bound ? dl::attn_dl_kernel<D, true> : dl::attn_dl_kernel<D, false>, dim3(grid),
-                           dim3(dl::kThreads), dl::Layout<D>::kTotal, stream, p, *tmap));
+        // Two instantiations of the one kernel, chosen per batch by the SURVEY.md 8(d) roofline formulas: HBM-bound
+        // batches run chunk tiles and decode streams side by side (dual lane); tensor-bound batches put both softmax
+        // warpgroups on every chunk tile (SPLIT) and move a quarter of the exponentials to the FMA pipe.
+        if (c->tensor_bound)
+            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, true, true>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, true>::kTotal, stream, p, *tmap));
+        else
+            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, false, false>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, false>::kTotal, stream, p, *tmap));
         CP_CUDA(cudaGetLastError());
         ++*launches;
         c->info.grid_attn = grid;
@@ -646,8 +659,10 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
             CP_CUDA(cudaGetLastError());
             ++launches;
             q = c->d_q_rot;
-        } else if (k_new) {
-            const int64_t total = (int64_t)m.n_tokens * c->shape.Hkv * (c->shape.D / 8) * 2;
+        } else {
+            // k_new == NULL (the caller wrote the pages): the kernel only zeroes the stale page tails
+            const int64_t total = std::max<int64_t>(k_new ? (int64_t)m.n_tokens * c->shape.Hkv * (c->shape.D / 8) * 2 : 0,
+                                                    (int64_t)m.n_reqs * 2 * c->shape.Hkv * (c->shape.B - 1) * (c->shape.D / 8));
             const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 8);
             kv_append_kernel<<<grid, 256, 0, stream>>>(m, c->shape, static_cast<const uint4*>(k_new),
                                                        static_cast<const uint4*>(v_new),

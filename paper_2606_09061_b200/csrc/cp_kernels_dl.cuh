@@ -27,6 +27,20 @@
 //               writes + one MMA read each).
 //   kKindSwap   <= 16 rows, D = 128: S^T[128 keys x 16] = K Q^T, O^T[128 d x 16] += V^T P^T.
 //
+//
+// SPLIT mode (template parameter; the instantiation the host launches for TENSOR-BOUND batches): there are no
+// decode streams worth a lane of their own, and a chunk tile is bound by its softmax (16 K exponentials, the
+// row maxima and sums of a 128 x 128 score tile on ONE warpgroup take ~2200 cycles against 1024 cycles of MMA).
+// So lane S's warpgroup joins lane T: the two softmax warpgroups split every score tile by COLUMNS -- warpgroup w
+// takes keys [64 w, 64 w + 64) of each 128-key tile for all 128 rows -- and exchange their row maxima through
+// shared memory (one 256-thread named barrier per tile), so both keep the same running reference maximum
+// without ever talking again; each keeps the partial row sum of its own columns and owns half of the O columns
+// for the (rare) rescale and for the epilogue.  Scores come as ONE N = 128 block per tile into one of two
+// 128-column S buffers (a tcgen05.mma has a ~50-cycle minimum: N = 64 blocks run at 51 cycles per instruction
+// against a 32-cycle floor, N = 128 blocks at their 64-cycle floor), PV as one K = 128 block; a
+// single issuer warp; all five producer warps feed one 6-slot ring.  Decode items of such a batch run after its
+// tile items on warpgroup 2 (swap kind).
+//
 // Operation: include/cp.h / DESIGN.md section 2.  Masking is by select, masked P is exactly 0.
 #pragma once
 #include <cuda.h>
@@ -40,7 +54,8 @@ namespace cp {
 namespace dl {
 
 constexpr int kThreads = 512;
-constexpr int kStagesT = 3, kStagesS = 3, kMaxStages = 4;
+constexpr int kStagesT = 3, kStagesS = 3, kMaxStages = 6;
+constexpr int kStagesSplit = 6, kProdSplit = 5;  // SPLIT mode: one ring, all five producer warps
 constexpr int kProdT = 3, kProdS = 2;         // TMA producer warps per lane (kProdT + kProdS + 3 MMA warps = 8 warps)
 // a producer waiting for slot reuse may be at most one phase behind only if kProd <= kStages
 static_assert(kProdT <= kStagesT && kProdS <= kStagesS && kProdT + kProdS == 5, "producer / stage configuration");
@@ -63,14 +78,16 @@ constexpr int kPolyEvery = DL_POLY_EVERY;
 constexpr float kRescaleThreshold = 8.0f;      // log2 units: rescale O only when the max grew > 2^8
 constexpr uint32_t kSmallBytes = 12288;        // per lane: Q^T (4 KiB) + double-buffered P^T (8 KiB)
 
-template <int D>
+template <int D, bool SPLIT = false>
 struct Layout {
     static constexpr int kHalves = D / 64;                    // 64-element (128-byte) halves of D
     static constexpr uint32_t kSlotBytes = kHalves * 16384;   // one K or V tile: 128 keys x D bf16
     // slot: [16 row groups][kHalves][8 rows][128 B] (one TMA box per page = 2 row groups)
     static constexpr uint32_t kGroupBytes = kHalves * 1024;   // UMMA SBO of a K/V slot
     static constexpr uint32_t kPageBytes = 2 * kGroupBytes;
-    static constexpr uint32_t kOffKv[2] = {0, kStagesT * kSlotBytes};
+    static constexpr int kStages = SPLIT ? kStagesSplit : kStagesT;     // of lane 0's ring
+    // SPLIT: the same 6 slots form ONE ring (lane 0); small[0] also holds the warpgroups' exchange arrays
+    static constexpr uint32_t kOffKv[2] = {0, SPLIT ? 0 : kStagesT * kSlotBytes};
     static constexpr uint32_t kOffSmall[2] = {(kStagesT + kStagesS) * kSlotBytes,
                                               (kStagesT + kStagesS) * kSlotBytes + kSmallBytes};
     static constexpr uint32_t kOffMisc = kOffSmall[1] + kSmallBytes;
@@ -164,14 +181,14 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
 // instruction footprint has to stay inside the 32 KB L1.5 instruction cache of the SM -- with one copy
 // per lane (and the other per-lane duplicates) it was 39 KB in a mixed batch and the tile softmax spent
 // 40-50 % of its issue slots waiting for instruction fetch (ncu: stall_no_inst; 4 % in a chunk-only batch).
-template <int D>
+template <int D, bool SPLIT>
 __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tmap, uint8_t* smem, Misc* misc, int lane, int warp) {
-    using L = Layout<D>;
+    using L = Layout<D, SPLIT>;
     static_assert(kStagesT == kStagesS, "the shared producer code assumes one ring depth");
-    constexpr int kStages = kStagesT;
-    const int LANE = warp < kProdT ? 0 : 1;
+    constexpr int kStages = L::kStages;
+    const int LANE = SPLIT ? 0 : (warp < kProdT ? 0 : 1);
     const int pw = LANE == 0 ? warp : warp - kProdT;
-    const int kProd = LANE == 0 ? kProdT : kProdS;
+    const int kProd = SPLIT ? kProdSplit : (LANE == 0 ? kProdT : kProdS);
     LaneState* ls = &misc->lane[LANE];
     constexpr uint32_t kOff0 = L::kOffKv[0], kOff1 = L::kOffKv[1];
     uint8_t* kv_base = smem + (LANE == 0 ? kOff0 : kOff1);
@@ -252,24 +269,6 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
     }
 }
 
-// Rows [first, 128) of the LAST V tile of an item are not keys of the request: slots of the last page
-// past kv_end hold whatever the pool held (another request's rows, NaN in a torch.empty pool), and
-// pages the tile does not have were never loaded (stale shared memory).  Masked P is exactly 0, but
-// 0 x NaN in the PV product is NaN, so the PV issuer zeroes those rows -- generic-proxy stores after
-// the TMA has landed, made visible to the tensor core's async proxy -- before it issues the block.
-// K needs nothing: a NaN score of a masked key is removed by select, never by arithmetic.
-template <int D>
-__device__ __forceinline__ void zero_v_tail(uint32_t v_tile, int first) {
-    using L = Layout<D>;
-    constexpr int kPerRow = L::kHalves * 8;                 // 16-byte chunks per key row
-    for (int i = first * kPerRow + (int)(threadIdx.x & 31); i < kKeyTile * kPerRow; i += 32) {
-        const int r = i / kPerRow, c = i % kPerRow;
-        ptx::st_shared_zero16(v_tile + (r >> 3) * L::kGroupBytes + (c >> 3) * 1024 + (r & 7) * 128 + (c & 7) * 16);
-    }
-    ptx::fence_proxy_async_smem();
-    __syncwarp();
-}
-
 // ------------------------------------------------------------------------------------------
 // MMA issuer warps (tcgen05.mma is issued by one elected thread; the warp stays convergent so
 // descriptors live in uniform registers).
@@ -331,10 +330,7 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
             const uint32_t ld = ld_base + (t == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * t + 2);
             const uint32_t slot = ld % kStages;
             ptx::mbar_wait(&ls->tp_full[buf], (g >> 2) & 1);
-            if (h == 0) {
-                ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
-                if (t == n_tiles - 1 && (n_keys & (kKeyTile - 1))) zero_v_tail<D>(kv_base + slot * L::kSlotBytes, n_keys & (kKeyTile - 1));
-            }
+            if (h == 0) ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
             ptx::tc_fence_after();
             const uint32_t v_half = kv_base + slot * L::kSlotBytes + h * 4 * L::kPageBytes;     // keys 64 h .. 64 h + 63
             const uint32_t d_tmem = tmem + col_o(0);
@@ -357,17 +353,81 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
     ld_base += 2 * n_tiles;
 }
 
-template <int D, int LANE, int ROLE>
-__device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
-                                         uint32_t& ld_base, uint32_t& gt, uint32_t& gp, uint32_t (&ic)[2], uint32_t& gpt) {
-    using L = Layout<D>;
-    constexpr int kStages = LANE == 0 ? kStagesT : kStagesS;
+// SPLIT mode, tile kind (one issuer warp): per 128-key tile t one score block QK(t) -- TS form, Q in TMEM, N = 128
+// keys, into S buffer (tile counter & 1) -- and one PV block over the whole tile once BOTH softmax warpgroups have
+// delivered their half of P(t) (tp_full counts their eight warps).  QK(t+1) is issued ahead of PV(t), so the next
+// scores wait for the warpgroups while the pipe runs PV(t); it overwrites the buffer PV(t-1) read: same thread,
+// program order, in-order pipe -- no barrier.  K-steps (pages) past the item's last key are not multiplied.
+template <int D>
+__device__ __forceinline__ void mma_split_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
+                                               uint32_t& ld_base, uint32_t& gt, uint32_t& ic) {
+    using L = Layout<D, true>;
+    constexpr int kStages = L::kStages;
     const int n_keys = __shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0);
     const int n_tiles = (n_keys + kKeyTile - 1) / kKeyTile;
+    const uint32_t kv_base = smem_base + L::kOffKv[0];
+    const uint32_t idesc_qk = ptx::umma_idesc_bf16(128, 128, false, false);
+    const uint32_t idesc_pv = ptx::umma_idesc_bf16(128, D, false, true);
+    const uint32_t g0 = gt;
+    ptx::mbar_wait(&ls->q_full[0], ic & 1);
+    ++ic;
+    ptx::tc_fence_after();
+    auto issue_qk = [&](int t) {
+        // load order of the producers: K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1)
+        const uint32_t ld = ld_base + (t == 0 ? 0 : 2 * t - 1);
+        const uint32_t slot = ld % kStages, buf = (g0 + t) & 1;
+        ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+        ptx::tc_fence_after();
+        if (ptx::elect_one()) {
+            const uint64_t k_desc0 = ptx::umma_desc_sw128(kv_base + slot * L::kSlotBytes, 16, L::kGroupBytes);
+#pragma unroll
+            for (int ks = 0; ks < D / 16; ++ks) {
+                const uint32_t koff = (ks >> 2) * 1024 + (ks & 3) * 32;            // K slot: halves of D 1 KB apart
+                umma_ts(tmem + buf * 128, tmem + kColQ + ks * 8, ptx::umma_desc_advance(k_desc0, koff), idesc_qk, ks > 0);
+            }
+            ptx::umma_commit(&ls->kv_empty[slot]);
+            ptx::umma_commit(&ls->ts_full[buf]);
+        }
+        __syncwarp();
+    };
+    issue_qk(0);
+    for (int t = 0; t < n_tiles; ++t) {
+        if (t + 1 < n_tiles) issue_qk(t + 1);
+        const uint32_t ld = ld_base + (t == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * t + 2);
+        const uint32_t slot = ld % kStages, g = g0 + t, buf = g & 1;
+        ptx::mbar_wait(&ls->tp_full[buf], (g >> 1) & 1);
+        ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+        ptx::tc_fence_after();
+        if (ptx::elect_one()) {
+            const uint64_t v_desc0 = ptx::umma_desc_sw128(kv_base + slot * L::kSlotBytes, 1024, L::kGroupBytes);
+#pragma unroll
+            for (int ks = 0; ks < kKeyTile / 16; ++ks) {
+                // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO).
+                // P of keys 64 w .. 64 w + 63 sits in the first 32 columns of half w of the S buffer.
+                if (t * kKeyTile + ks * 16 < n_keys)
+                    umma_ts(tmem + col_o(0), tmem + buf * 128 + (ks >> 2) * 64 + (ks & 3) * 8,
+                            ptx::umma_desc_advance(v_desc0, ks * L::kPageBytes), idesc_pv, t > 0 || ks > 0);
+            }
+            ptx::umma_commit(&ls->kv_empty[slot]);
+            ptx::umma_commit(&ls->tpv_done[buf]);
+        }
+        __syncwarp();
+    }
+    gt += n_tiles;
+    ld_base += 2 * n_tiles;
+}
+
+template <int D, int LANE, int ROLE, bool SPLIT>
+__device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
+                                         uint32_t& ld_base, uint32_t& gt, uint32_t& gp, uint32_t (&ic)[2], uint32_t& gpt) {
+    using L = Layout<D, SPLIT>;
+    constexpr int kStages = SPLIT ? L::kStages : (LANE == 0 ? kStagesT : kStagesS);
+    const int n_tiles = (__shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0) + kKeyTile - 1) / kKeyTile;
     const bool swap = LANE == 1 || __shfl_sync(0xffffffffu, it.kind, 0) == kKindSwap;
     const bool all = ROLE == 0 || swap;        // this warp issues both kinds of block
     if (!swap) {
-        if constexpr (LANE == 0 && ROLE != 0) mma_tile_item<D, ROLE>(it, smem_base, ls, tmem, ld_base, gpt, ic);
+        if constexpr (SPLIT) mma_split_item<D>(it, smem_base, ls, tmem, ld_base, gpt, ic[0]);
+        else if constexpr (LANE == 0 && ROLE != 0) mma_tile_item<D, ROLE>(it, smem_base, ls, tmem, ld_base, gpt, ic);
         return;
     }
     if (ROLE == 2) {                           // swap item on lane T: ROLE 1 issues it; stay in step
@@ -425,9 +485,8 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
         ptx::mbar_wait(&ls->p_full[set][gp & 1], (gp >> 1) & 1);
         ++gp;
         ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
-        const uint32_t v_tile = kv_base + slot * L::kSlotBytes;
-        if (t == n_tiles - 1 && (n_keys & (kKeyTile - 1))) zero_v_tail<D>(v_tile, n_keys & (kKeyTile - 1));
         ptx::tc_fence_after();
+        const uint32_t v_tile = kv_base + slot * L::kSlotBytes;
         const uint32_t d_tmem = tmem + col_o(LANE);
         if (ptx::elect_one()) {
             const uint64_t v_desc0 = ptx::umma_desc_sw128(v_tile, 1024, L::kGroupBytes);
@@ -463,7 +522,7 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
     ld_base += 2 * n_tiles;
 }
 
-template <int D, int LANE, int ROLE>
+template <int D, int LANE, int ROLE, bool SPLIT>
 __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lane) {
     LaneState* ls = &misc->lane[LANE];
     const uint32_t tmem = misc->tmem_base;
@@ -475,7 +534,7 @@ __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lan
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&ls->item_empty[islot]);
         if (it.kind < 0) break;
-        mma_item<D, LANE, ROLE>(it, smem_base, ls, tmem, ld_base, gt, gp, ic, gpt);
+        mma_item<D, LANE, ROLE, SPLIT>(it, smem_base, ls, tmem, ld_base, gt, gp, ic, gpt);
         ++item_cnt;
     }
 }
@@ -621,6 +680,160 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
 }
 
 // ------------------------------------------------------------------------------------------
+// SPLIT mode: softmax of warpgroup w (0 / 1) for a chunk tile: thread <-> row of the 128-row Q tile, columns
+// (keys) [64 w, 64 w + 64) of every 128-key score tile.  Per tile: the half score row from TMEM, its maximum,
+// the exchange of the two half-row maxima through shared memory (one 256-thread named barrier), then both
+// threads of a row take the SAME decision about the reference maximum (lazy rescale: only when the row maximum
+// grew by more than 2^8), exponentials, partial row sum of the own columns, P (bf16 pairs) back over the scores
+// of the own half.  Warpgroup w owns O columns [w D/2, (w + 1) D/2) for the rescale and the epilogue; the two
+// partial row sums meet in shared memory at the end.  Warpgroup 0 puts the Q tile into TMEM.
+// ------------------------------------------------------------------------------------------
+template <int D, bool POLY>
+__device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& p, LaneState* ls, uint32_t tmem, uint8_t* xchg,
+                                              uint32_t& gt, int row, uint32_t lane_base, int w) {
+    const Shape& sh = p.sh;
+    const int G = sh.G;
+    const int gs = 31 - __clz(G);                        // G is a power of two (cp_create): shifts, not divisions
+    const int R = it.q_tokens * G;
+    const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
+    const int tok0 = p.meta.cu_q[it.req] + it.q_start;
+    const int ctx = p.meta.ctx_off[it.req];
+    const bool valid_row = row < R;
+    const int tok = tok0 + (row >> gs);
+    const int head = it.kv_head * G + (row & (G - 1));
+    const float scale = sh.sm_scale * 1.4426950408889634f;
+    const uint32_t t_row = tmem + (lane_base << 16);
+    const uint32_t c_o = col_o(0) + w * (D / 2);         // this warpgroup's half of the O columns
+    float* xmax = reinterpret_cast<float*>(xchg);        // [tile parity][warpgroup][row]: half-row maxima (raw scores)
+    float* xl = xmax + 512;                              // [warpgroup][row]: partial row sums
+
+    if (w == 0) {
+        // ---- Q row -> TMEM (A operand of QK^T): column j holds elements (2j, 2j+1)
+        const uint4* src = reinterpret_cast<const uint4*>(p.q + ((int64_t)tok * sh.Hq + head) * D);
+#pragma unroll
+        for (int c = 0; c < D / 64; ++c) {
+            uint32_t r[32];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const uint4 v = valid_row ? src[c * 8 + j] : make_uint4(0, 0, 0, 0);
+                r[4 * j] = v.x; r[4 * j + 1] = v.y; r[4 * j + 2] = v.z; r[4 * j + 3] = v.w;
+            }
+            ptx::tmem_st32(t_row + kColQ + c * 32, r);
+        }
+        ptx::tmem_wait_st();
+        ptx::tc_fence_before();
+        warp_arrive(&ls->q_full[0]);
+    }
+
+    const int limit = valid_row ? min(it.kv_end, ctx + it.q_start + (row >> gs) + 1) : 0;   // causal, diagonal inclusive
+    float m_ref = -INFINITY, l = 0.f;
+
+    for (int t = 0; t < n_tiles; ++t) {
+        const int ts = it.kv_begin + t * kKeyTile + w * 64;
+        const uint32_t buf = gt & 1;
+        const uint32_t t_s = t_row + buf * 128 + w * 64;
+        ptx::mbar_wait(&ls->ts_full[buf], (gt >> 1) & 1);
+        ptx::tc_fence_after();
+        uint32_t sr[64];
+        ptx::tmem_ld32(t_s, sr);
+        ptx::tmem_ld32(t_s + 32, sr + 32);
+        ptx::tmem_wait_ld();
+        const int nvalid = max(0, min(64, limit - ts));
+        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};      // independent max chains
+        if (nvalid == 64) {
+#pragma unroll
+            for (int i = 0; i < 64; ++i) mx[i & 3] = fmaxf(mx[i & 3], __uint_as_float(sr[i]));
+        } else {
+#pragma unroll
+            for (int i = 0; i < 64; ++i) mx[i & 3] = fmaxf(mx[i & 3], i < nvalid ? __uint_as_float(sr[i]) : -INFINITY);
+        }
+        const float m_loc = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+        xmax[(gt & 1) * 256 + w * 128 + row] = m_loc;
+        ptx::named_bar_sync(3, 256);                     // both warpgroups: the other half's maximum is there
+        const float m_t = fmaxf(m_loc, xmax[(gt & 1) * 256 + (w ^ 1) * 128 + row]) * scale;     // scale > 0
+        float alpha = 1.f;
+        bool rescale = false;
+        if (m_t > m_ref + kRescaleThreshold) {          // also the first finite max (m_ref = -inf)
+            alpha = (m_ref == -INFINITY) ? 0.f : ptx::ex2(m_ref - m_t);
+            m_ref = m_t;
+            rescale = true;
+        }
+        const float neg_m = (m_ref == -INFINITY) ? 0.f : -m_ref;
+        float sm[4] = {0.f, 0.f, 0.f, 0.f};             // independent sum chains
+        uint32_t pk[32];                                // 64 scores -> 32 packed P columns
+        if (nvalid == 64) {
+#pragma unroll
+            for (int i = 0; i < 64; i += 2) {
+                const float a = ex2_sel<POLY>(fmaf(__uint_as_float(sr[i]), scale, neg_m), i);
+                const float b = ex2_sel<POLY>(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1);
+                sm[(i >> 1) & 3] += a + b;
+                pk[i >> 1] = pack_bf16(a, b);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 64; i += 2) {
+                const float a = i < nvalid ? ex2_sel<POLY>(fmaf(__uint_as_float(sr[i]), scale, neg_m), i) : 0.f;
+                const float b = i + 1 < nvalid ? ex2_sel<POLY>(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1) : 0.f;
+                sm[(i >> 1) & 3] += a + b;
+                pk[i >> 1] = pack_bf16(a, b);
+            }
+        }
+        ptx::tmem_st32(t_s, pk);
+        l = l * alpha + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
+        // same rows, same m_t, same m_ref in warp k of both warpgroups: the same decision on both sides
+        if (t > 0 && __any_sync(0xffffffffu, rescale)) {
+            ptx::mbar_wait(&ls->tpv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);      // PV(t-1) (and all before) done: O readable
+            ptx::tc_fence_after();
+#pragma unroll 1
+            for (int c = 0; c < D / 64; ++c) {
+                uint32_t o[32];
+                ptx::tmem_ld32(t_row + c_o + c * 32, o);
+                ptx::tmem_wait_ld();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                ptx::tmem_st32(t_row + c_o + c * 32, o);
+            }
+        }
+        ptx::tmem_wait_st();
+        ptx::tc_fence_before();
+        warp_arrive(&ls->tp_full[buf]);
+        ++gt;
+    }
+
+    // ---- epilogue: this warpgroup's half of the O row -> out (bf16, normalised) or split workspace (fp32, unnormalised)
+    ptx::mbar_wait(&ls->tpv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
+    ptx::tc_fence_after();
+    xl[w * 128 + row] = l;
+    ptx::named_bar_sync(3, 256);
+    l += xl[(w ^ 1) * 128 + row];
+    const float inv = 1.f / l;
+#pragma unroll 1
+    for (int c = 0; c < D / 64; ++c) {
+        uint32_t o[32];
+        ptx::tmem_ld32(t_row + c_o + c * 32, o);
+        ptx::tmem_wait_ld();
+        if (!valid_row) continue;
+        const int d0 = w * (D / 2) + c * 32;
+        if (it.partial_row < 0) {
+            uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * sh.Hq + head) * D + d0);
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                dst[j] = make_uint4(pack_bf16(__uint_as_float(o[8 * j]) * inv, __uint_as_float(o[8 * j + 1]) * inv),
+                                    pack_bf16(__uint_as_float(o[8 * j + 2]) * inv, __uint_as_float(o[8 * j + 3]) * inv),
+                                    pack_bf16(__uint_as_float(o[8 * j + 4]) * inv, __uint_as_float(o[8 * j + 5]) * inv),
+                                    pack_bf16(__uint_as_float(o[8 * j + 6]) * inv, __uint_as_float(o[8 * j + 7]) * inv));
+        } else {
+            uint4* dst = reinterpret_cast<uint4*>(p.part_o + ((int64_t)it.partial_row + row) * D + d0);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) dst[j] = make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+        }
+    }
+    if (w == 0 && valid_row && it.partial_row >= 0) p.part_ml[(int64_t)it.partial_row + row] = make_float2(m_ref, l);
+    ptx::tc_fence_before();
+    ptx::named_bar_sync(3, 256);                         // the exchange arrays are reused by the next item
+}
+
+// ------------------------------------------------------------------------------------------
 // softmax warps, swap kind (D = 128, R <= RC <= 16 rows): thread <-> key of the tile (S^T lane)
 // during the key loop, thread <-> d (O^T lane) for rescale / epilogue.  Column c = (token, head)
 // row; columns in [R, RC) are computed as fully masked.  Straight-line code per column so the
@@ -761,10 +974,12 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
 
 // softmax warpgroup loop.  ROLE 0: lane T (tile kind, and the swap-kind items lane T picks up);
 // ROLE 2: lane S.
-template <int D, int ROLE, bool POLY>
+// SPLIT: both warpgroups follow lane 0's item ring; ROLE 0 = warpgroup 0 of the column split (and the swap-kind
+// items), ROLE 2 = warpgroup 1 (swap-kind items are skipped).
+template <int D, int ROLE, bool POLY, bool SPLIT>
 __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Misc* misc, int warp, int lane) {
-    using L = Layout<D>;
-    constexpr int LANE = ROLE == 2 ? 1 : 0;
+    using L = Layout<D, SPLIT>;
+    constexpr int LANE = (ROLE == 2 && !SPLIT) ? 1 : 0;
     LaneState* ls = &misc->lane[LANE];
     const uint32_t tmem = misc->tmem_base;
     const uint32_t lane_base = (warp & 3) * 32;
@@ -777,6 +992,14 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
         const WorkItem it = ls->items[islot];
         warp_arrive(&ls->item_empty[islot]);
         if (it.kind < 0) break;
+        if constexpr (SPLIT) {
+            if (it.kind == kKindTile) {
+                softmax_split<D, POLY>(it, p, ls, tmem, small, gh_tile, row, lane_base, ROLE == 2 ? 1 : 0);
+                ++item_cnt;
+                continue;
+            }
+            if (ROLE == 2) { ++item_cnt; continue; }
+        }
         if (ROLE == 2 || it.kind == kKindSwap) {
             if constexpr (D == 128) {
                 const int R = it.q_tokens * p.sh.G;
@@ -785,7 +1008,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
                 else softmax_swap<LANE, 16>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
             }
         } else {
-            if constexpr (ROLE == 0) softmax_tile<D, POLY>(it, p, ls, tmem, gh_tile, row, lane_base);
+            if constexpr (ROLE == 0 && !SPLIT) softmax_tile<D, POLY>(it, p, ls, tmem, gh_tile, row, lane_base);
         }
         ++item_cnt;
     }
@@ -794,10 +1017,10 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
 // ------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------
-template <int D, bool POLY>
+template <int D, bool POLY, bool SPLIT>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
-    using L = Layout<D>;
+    using L = Layout<D, SPLIT>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     Misc* misc = reinterpret_cast<Misc*>(smem + L::kOffMisc);
@@ -817,19 +1040,25 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             for (int i = 0; i < 4; ++i) {
                 ptx::mbar_init(&ls->ts_full[i], 1);
-                ptx::mbar_init(&ls->tp_full[i], 4);
+                ptx::mbar_init(&ls->tp_full[i], SPLIT ? 8 : 4);      // SPLIT: both warpgroups deliver a half of P
                 ptx::mbar_init(&ls->tpv_done[i], 1);
                 ptx::mbar_init(&ls->pv_issued[i], 1);
             }
             // readers of the item ring (one arrival per warp): the lane's 4 softmax warps, its MMA warp(s), its other producers
-            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], 4 + (ln == 0 ? 2 + kProdT - 1 : 1 + kProdS - 1)); }
+            // (SPLIT: one ring for everybody -- 8 softmax warps, 1 issuer, the other producers)
+            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], SPLIT ? 8 + 1 + kProdSplit - 1 : 4 + (ln == 0 ? 2 + kProdT - 1 : 1 + kProdS - 1)); }
         }
         ptx::fence_barrier_init();
         ptx::prefetch_tmap(&tmap);
     }
     if (warp == 6) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
-    // shared memory is NOT cleared: nothing stale in it can reach a result (masked scores are removed by
-    // select, the rows of a V tile past the item's last key are zeroed by the PV issuer, zero_v_tail)
+    // Stale shared memory may hold NaN bit patterns, tiles are only partly overwritten by short requests, and
+    // masked P = 0 times a NaN V row would poison the accumulators.  After this clear everything that ever sits
+    // in the ring is finite: K/V rows that are keys of their request, page tails that the append kernel zeroed
+    // (cp_kernels_simt.cuh), or these zeros.
+    for (uint32_t i = threadIdx.x * 16; i < L::kOffMisc; i += kThreads * 16)
+        *reinterpret_cast<uint4*>(smem + i) = make_uint4(0, 0, 0, 0);
+    ptx::fence_proxy_async_smem();
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
@@ -841,16 +1070,17 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     // their share to the tile softmax (a 128-column score row in registers) and the decode softmax.
     if (warp < 8) {
         reg_dec<56>();
-        if (warp < kProdT + kProdS) producer<D>(p, &tmap, smem, misc, lane, warp);
-        else if (warp == 5) mma_warp<D, 0, 1>(ptx::smem_u32(smem), misc, lane);      // lane T: score blocks (and swap items)
-        else if (warp == 6) mma_warp<D, 0, 2>(ptx::smem_u32(smem), misc, lane);      // lane T: PV blocks
-        else mma_warp<D, 1, 0>(ptx::smem_u32(smem), misc, lane);                     // lane S
+        if (warp < kProdT + kProdS) producer<D, SPLIT>(p, &tmap, smem, misc, lane, warp);
+        else if (warp == 5) mma_warp<D, 0, 1, SPLIT>(ptx::smem_u32(smem), misc, lane);     // lane T: score blocks (and swap items); SPLIT: the one issuer
+        else if (SPLIT) { }                                                                 // SPLIT: warps 6, 7 have no role
+        else if (warp == 6) mma_warp<D, 0, 2, false>(ptx::smem_u32(smem), misc, lane);     // lane T: PV blocks
+        else mma_warp<D, 1, 0, false>(ptx::smem_u32(smem), misc, lane);                    // lane S
     } else if (warp < 12) {
-        reg_inc<232>();
-        softmax_warps<D, 0, POLY>(p, smem, misc, warp, lane);
+        reg_inc<SPLIT ? 200 : 232>();
+        softmax_warps<D, 0, POLY, SPLIT>(p, smem, misc, warp, lane);
     } else {
-        reg_inc<160>();
-        softmax_warps<D, 2, false>(p, smem, misc, warp, lane);
+        reg_inc<SPLIT ? 200 : 160>();
+        softmax_warps<D, 2, SPLIT && POLY, SPLIT>(p, smem, misc, warp, lane);
     }
     ptx::tc_fence_before();
     __syncthreads();

@@ -17,13 +17,46 @@ __device__ __forceinline__ int64_t slab_elem_offset(int64_t page, int kv, int he
 }
 
 // ---------------------------------------------------------------------------------
-// H2: one thread per 16-byte chunk of a (token, kv head, K|V) row.
+// Stale page tails.  The attention kernel moves whole 16-token page slabs with TMA and masks the scores
+// of slots that are not keys by select; but masked P = 0 still multiplies the V row of such a slot in the
+// tensor-core PV product, and 0 x NaN is NaN.  So every step zeroes, for every request of the batch, the
+// slots of its LAST page that lie past its last key (<= 15 slots x Hkv x K|V): they belong to the request,
+// hold no key, and later appends overwrite them.  (K tails too: a K tile's stale rows can be left in a ring
+// slot that a shorter V tile later only partly overwrites.)  With that and the kernel's prologue clear, a
+// torch.empty pool or NaN-filled tails cannot reach a result (include/cp.h; reading R6).
+// One thread per 16-byte chunk of a (request, K|V, kv head, slot 1..15) row; most exit at once.
+// ---------------------------------------------------------------------------------
+__device__ __forceinline__ void zero_page_tails(const BatchMeta& meta, const Shape& sh, __nv_bfloat16* __restrict__ cache) {
+    const int chunks = sh.D / 8;
+    const int64_t total = (int64_t)meta.n_reqs * 2 * sh.Hkv * (sh.B - 1) * chunks;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int c = (int)(i % chunks);
+        int64_t r = i / chunks;
+        const int slot = 1 + (int)(r % (sh.B - 1));
+        r /= (sh.B - 1);
+        const int g = (int)(r % sh.Hkv);
+        r /= sh.Hkv;
+        const int kv = (int)(r & 1);
+        const int req = (int)(r >> 1);
+        const int last = meta.ctx_off[req] + meta.q_len[req] - 1;       // position of the request's last key
+        if (slot <= last % sh.B) continue;
+        const int64_t page = meta.block_table[meta.bt_off[req] + last / sh.B];
+        __nv_bfloat16* dst = cache + slab_elem_offset(page, kv, g, sh.Hkv, sh.B, sh.D) + (int64_t)slot * sh.D + c * 8;
+        *reinterpret_cast<uint4*>(dst) = make_uint4(0, 0, 0, 0);
+    }
+}
+
+// ---------------------------------------------------------------------------------
+// H2: one thread per 16-byte chunk of a (token, kv head, K|V) row; then the page tails (above).
+// k_new == nullptr (the caller wrote the pages itself): only the page tails.
 // ---------------------------------------------------------------------------------
 __global__ void kv_append_kernel(BatchMeta meta, Shape sh, const uint4* __restrict__ k_new,
                                  const uint4* __restrict__ v_new, __nv_bfloat16* __restrict__ cache) {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the attention kernel may start its prologue
+    zero_page_tails(meta, sh, cache);
     const int chunks = sh.D / 8;                          // 16-byte chunks per row
-    const int64_t total = (int64_t)meta.n_tokens * sh.Hkv * chunks * 2;
+    const int64_t total = k_new ? (int64_t)meta.n_tokens * sh.Hkv * chunks * 2 : 0;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
          i += (int64_t)gridDim.x * blockDim.x) {
         int c = (int)(i % chunks);
@@ -92,6 +125,7 @@ __global__ void kv_append_rope_kernel(BatchMeta meta, Shape sh, const uint4* __r
                                       const float2* __restrict__ cs, __nv_bfloat16* __restrict__ cache,
                                       uint4* __restrict__ q_rot) {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the attention kernel may start its prologue
+    zero_page_tails(meta, sh, cache);
     const int chunks = sh.D / 8, hc = sh.D / 16, half = sh.D / 2;
     const int v_units = sh.Hkv * chunks;
     const int per_tok = v_units + (sh.Hkv + sh.Hq) * hc;

@@ -83,3 +83,28 @@ def sample_rows(spec, n, seed=0):
     tok = np.concatenate([tok, extra]).astype(np.int64)
     head = rng.integers(0, spec.Hq, size=len(tok)).astype(np.int32)
     return tok, head
+
+
+def keys_per_page(spec) -> np.ndarray:
+    """For every page in touched_pages() order: how many of its 16 slots hold a key of its request AFTER the step."""
+    out = []
+    for bt, q, o in zip(spec.block_tables, spec.q_len, spec.ctx_off):
+        kv_len = int(q) + int(o)
+        out.append(np.clip(kv_len - np.arange(len(bt)) * spec.B, 0, spec.B))
+    return np.concatenate(out).astype(np.int64) if out else np.zeros(0, np.int64)
+
+
+def assert_pages(got, want, nk, what="pages"):
+    """H2 parity on pages [n, 2, Hkv, B, D] (bit patterns): every slot that holds a key equals the oracle's append
+    bit for bit; the slots of a request's last page past its last key are ZERO (the step clears them, include/cp.h:
+    they hold no key); every other slot is untouched (= the oracle's copy, which never writes there)."""
+    B = got.shape[3]
+    slot = np.arange(B)[None, :]
+    is_key = slot < nk[:, None]                                        # [n, B]
+    is_tail = (~is_key) & (nk[:, None] > 0)                            # partly filled page = the request's last page
+    k4 = is_key[:, None, None, :, None]
+    t4 = is_tail[:, None, None, :, None]
+    assert np.array_equal(np.where(k4, got, 0), np.where(k4, want, 0)), f"{what}: appended rows differ from the oracle's append"
+    assert not np.where(t4, got, 0).any(), f"{what}: slots past the last key of a last page are not zero"
+    o4 = ~(k4 | t4)
+    assert np.array_equal(np.where(o4, got, 0), np.where(o4, want, 0)), f"{what}: a slot outside the batch's key range was modified"

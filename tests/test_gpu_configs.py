@@ -30,8 +30,9 @@ def _run_device_config(spec, variant, n_sample):
     # H2 parity: the pages the step wrote equal the oracle's append, bit for bit
     touched = torch.from_numpy(spec.touched_pages().astype(np.int64)).to(dev)
     step = 8192
+    nk = gu.keys_per_page(spec)
     for s in range(0, len(touched), step):
-        assert np.array_equal(gu.to_bits(pool[touched[s:s + step]]), cache[s:s + step])
+        gu.assert_pages(gu.to_bits(pool[touched[s:s + step]]), cache[s:s + step], nk[s:s + step])
     if n_sample is None:
         want = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale)
         stats = gu.assert_close(got, want, spec.name)

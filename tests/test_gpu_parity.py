@@ -19,8 +19,10 @@ def test_tiny_config_full(variant):
     got, pool_after = gu.run_gpu_host_values(spec, hv, variant)
     want, cache_after = gu.run_oracle_host_values(spec, hv)
     gu.assert_close(got, want, "tiny")
-    # H2: the appended pages are bit-identical to the oracle's append; nothing else moved
-    assert np.array_equal(pool_after[spec.touched_pages()], cache_after)
+    # H2: the appended rows are bit-identical to the oracle's append; last-page tails are cleared; nothing else moved
+    gu.assert_pages(pool_after[spec.touched_pages()], cache_after, gu.keys_per_page(spec))
+    untouched = np.setdiff1d(np.arange(spec.num_blocks), spec.touched_pages())
+    assert np.array_equal(pool_after[untouched], wl.full_pool_from_compact(spec, hv.cache)[untouched])
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -77,11 +79,12 @@ def test_stale_tails_nan_strict(Hq, Hkv, D, q_len, ctx_off):
         got_nan, pool_after = gu.run_gpu_host_values(spec, hv_nan, 0, append=append, poison=wl.NAN_BF16)
         gu.assert_close(got_nan, want, f"NaN tails, append={append}")
         assert np.array_equal(got_nan, got_fin)
-    # the NaN really was there: slots past kv_len of a request's last page still hold it after the step
-    j = int(np.argmax((spec.ctx_off + spec.q_len) % 16 != 0))
-    kv_len = int(spec.ctx_off[j] + spec.q_len[j])
-    last = pool_after[spec.block_tables[j][(kv_len - 1) // 16]]
-    assert (last[:, :, kv_len % 16:, :] == (wl.NAN_BF16, wl.NAN_BF16 ^ 0x8000)[((kv_len - 1) // 16) & 1]).all()
+    # the NaN really was there: the pool's untouched pages still hold it after the step; the tails of the requests'
+    # last pages were cleared by the step (they hold no key)
+    untouched = np.setdiff1d(np.arange(spec.num_blocks), spec.touched_pages())
+    assert ((pool_after[untouched] & 0x7FFF) == wl.NAN_BF16).all()
+    _, cache_after = gu.run_oracle_host_values(spec, hv_nan)
+    gu.assert_pages(pool_after[spec.touched_pages()], cache_after, gu.keys_per_page(spec))
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -240,7 +243,7 @@ def test_fuzz_shapes_against_oracle(seed):
     got, pool_after = gu.run_gpu_host_values(spec, hv, 0)
     want, cache_after = gu.run_oracle_host_values(spec, hv)
     gu.assert_close(got, want, spec.name)
-    assert np.array_equal(pool_after[spec.touched_pages()], cache_after)
+    gu.assert_pages(pool_after[spec.touched_pages()], cache_after, gu.keys_per_page(spec))
 
 
 def test_repeated_launches_mixed_shapes_no_deadlock():
@@ -298,3 +301,35 @@ def test_tensor_bound_batches_take_the_fma_pipe_share_kernel(Hq, Hkv, D, q_len, 
     tok, head = gu.sample_rows(spec2, 256, seed=3)
     want2, _ = gu.run_oracle_host_values(spec2, hv2, rows=(tok, head))
     gu.assert_close(got2[tok, head], want2, "hbm-bound batch")
+
+
+SPLIT_CASES = [
+    # (Hq, Hkv, D, q_len, ctx_off): every batch is tensor-bound by the SURVEY.md 8(d) formulas -> SPLIT instantiation
+    (8, 2, 128, [1200], [0]),                      # G = 4: a pair is 2 x 32 tokens; 18.75 pairs -> last pair's second tile empty
+    (8, 2, 128, [1376, 673], [200, 1000]),         # odd numbers of Q tiles, ragged key ranges
+    (8, 2, 128, [579, 769], [5, 777]),             # remainders: a 3-token tail (12 rows -> swap-kind item on the TWIN kernel)
+    (2, 2, 128, [2600], [100]),                    # G = 1: a pair is 256 tokens
+    (16, 1, 128, [700, 663], [0, 3000]),           # G = 16: a pair is 16 tokens
+    (16, 2, 64, [1300, 900], [1000, 0]),           # D = 64 (tile kind only), G = 8
+    (8, 2, 128, [100], [30000]),                   # long context: the pair's key range is split over the SMs + combine
+    (32, 8, 128, [384, 1, 1, 1], [2048, 300, 17, 4000]),   # 8B shape with a few short decodes (swap items after the tiles)
+    (64, 8, 128, [200, 1], [5000, 12000]),         # 70B shape, G = 8
+    (8, 2, 128, [1000, 65], [64, 0]),              # last tile of <= 64 keys (phantom second half), 1-token remainder
+]
+
+
+@pytest.mark.parametrize("Hq,Hkv,D,q_len,ctx_off", SPLIT_CASES)
+def test_split_mode_tensor_bound_batches(Hq, Hkv, D, q_len, ctx_off):
+    """Tensor-bound batches run the SPLIT instantiation (both softmax warpgroups on every chunk tile):
+    full oracle comparison, NaN in every stale slot, pages bit-exact; cp_get_batch_info confirms the mode."""
+    pages = sum((q + o + 15) // 16 for q, o in zip(q_len, ctx_off)) + 11
+    spec = wl.make_spec("split", Hq, Hkv, D, 16, pages, q_len, ctx_off, seed=41)
+    hv = wl.host_values(spec, poison=wl.NAN_BF16)
+    ctx = gu.make_ctx(spec)
+    got, pool_after = gu.run_gpu_host_values(spec, hv, 0, ctx=ctx, poison=wl.NAN_BF16)
+    assert ctx.cp_get_batch_info().split == 1
+    ctx.close()
+    want, cache_after = gu.run_oracle_host_values(spec, wl.host_values(spec))
+    gu.assert_close(got, want, "split")
+    _, cache_nan = gu.run_oracle_host_values(spec, hv)
+    gu.assert_pages(pool_after[spec.touched_pages()], cache_nan, gu.keys_per_page(spec))
