@@ -33,7 +33,7 @@
 // row maxima and sums of a 128 x 128 score tile on ONE warpgroup take ~2200 cycles against 1024 cycles of MMA).
 // So lane S's warpgroup joins lane T: the two softmax warpgroups split every score tile by COLUMNS -- warpgroup w
 // takes keys [64 w, 64 w + 64) of each 128-key tile for all 128 rows -- and exchange their row maxima through
-// shared memory (one 256-thread named barrier per tile), so both keep the same running reference maximum
+// shared memory (one named barrier per tile and pair of warps that hold the same rows), so both keep the same running reference maximum
 // without ever talking again; each keeps the partial row sum of its own columns and owns half of the O columns
 // for the (rare) rescale and for the epilogue.  Scores come as ONE N = 128 block per tile into one of two
 // 128-column S buffers (a tcgen05.mma has a ~50-cycle minimum: N = 64 blocks run at 51 cycles per instruction
@@ -749,7 +749,7 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
         }
         const float m_loc = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
         xmax[(gt & 1) * 256 + w * 128 + row] = m_loc;
-        ptx::named_bar_sync(3, 256);                     // both warpgroups: the other half's maximum is there
+        ptx::named_bar_sync(3 + (int)(lane_base >> 5), 64);   // this warp and its partner (same rows, other half): its maxima are there
         const float m_t = fmaxf(m_loc, xmax[(gt & 1) * 256 + (w ^ 1) * 128 + row]) * scale;     // scale > 0
         float alpha = 1.f;
         bool rescale = false;
@@ -804,7 +804,7 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
     ptx::mbar_wait(&ls->tpv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
     ptx::tc_fence_after();
     xl[w * 128 + row] = l;
-    ptx::named_bar_sync(3, 256);
+    ptx::named_bar_sync(3 + (int)(lane_base >> 5), 64);
     l += xl[(w ^ 1) * 128 + row];
     const float inv = 1.f / l;
 #pragma unroll 1
@@ -830,7 +830,7 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
     }
     if (w == 0 && valid_row && it.partial_row >= 0) p.part_ml[(int64_t)it.partial_row + row] = make_float2(m_ref, l);
     ptx::tc_fence_before();
-    ptx::named_bar_sync(3, 256);                         // the exchange arrays are reused by the next item
+    ptx::named_bar_sync(3 + (int)(lane_base >> 5), 64);  // the exchange arrays are reused by the next item
 }
 
 // ------------------------------------------------------------------------------------------
