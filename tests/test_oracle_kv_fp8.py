@@ -79,9 +79,10 @@ def test_round_trip_properties():
     err = np.abs(back - x)
     bound = np.maximum(np.abs(x) * 2.0 ** -4, 2.0 ** -10 * 2.0 ** e.astype(np.float64)[..., None])
     assert np.all(err <= bound)
-    # idempotent: quantising the dequantised row reproduces codes and scale
+    # idempotent in value: the dequantised row is a fixed point (codes / scale may shift by one binade when the
+    # row maximum rounded down to 224)
     codes2, e2 = q8.quantize_rows(back)
-    assert np.array_equal(codes2, codes) and np.array_equal(e2, e)
+    assert np.array_equal(q8.dequantize(codes2, e2), back)
     # exact in bf16 (hence the attention oracle can take the pages as bf16 bit patterns)
     bits = q8.f64_to_bf16_bits_exact(back)
     assert np.array_equal(wl.bf16_bits_to_f64(bits), back)
