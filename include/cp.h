@@ -71,7 +71,15 @@ typedef struct {
     int32_t kernel_variant;   /* must be 0.  (Library builds with -DCP_DEBUG_VARIANTS also
                                  accept 1 = a SIMT cross-check kernel for bisecting; the
                                  shipped library holds one attention kernel and rejects it.) */
+    int32_t kv_dtype;         /* CP_KV_BF16 (0) or CP_KV_E4M3 (1): format of the KV pool.  E4M3
+                                 pools are driven through cp_attention_step_fp8 (D = 128 only) */
+    int32_t reserved;         /* must be 0                                          */
+    int64_t max_scratch_pages;/* CP_KV_E4M3 only: pages of the library's bf16 scratch pool that
+                                 holds, per step, the dequantised pages of the requests with a
+                                 prefill chunk (> 8 rows per KV head); 0 = max_total_pages */
 } cp_config;
+#define CP_KV_BF16 0
+#define CP_KV_E4M3 1
 
 /* One request of the iteration.  HOST pointers. */
 #define CP_REQ_PREFILL 1         /* flags: this request is in its prefill phase   */
@@ -163,6 +171,25 @@ int cp_attention_step(cp_ctx* ctx, int32_t layer, const void* q, const void* k_n
 int cp_enable_rope(cp_ctx* ctx, const double* inv_freq);
 int cp_attention_step_rope(cp_ctx* ctx, int32_t layer, const void* q, const void* k_new,
                            const void* v_new, void* kv_cache, void* out, void* cuda_stream);
+
+/* N2 of SURVEY.md 8(f), second half: FP8 (e4m3) KV pages -- half the bytes of the memory-bound decode
+ * streams ("decode ... memory-bandwidth-bound").  PAPER.md defines none of it; DESIGN.md
+ * R13-R15.  Pool layout (ABI), one pool per layer:
+ *     kv_cache8[block][kv: 0 = K, 1 = V][kv_head][slot 0..B-1][d 0..D-1]   uint8, OCP FP8 E4M3 codes
+ *     kv_scale [block][kv][kv_head][slot]                                  float32, a power of two 2^e
+ * The value a slot holds is code_value * 2^e exactly.  Appended rows are quantised row by row: e = the smallest
+ * integer with 448 * 2^e >= amax(row), clamped to [-15, 7]; code = round-to-nearest-even of x * 2^-e, saturating
+ * at +-448 (oracle/kv_fp8.py is the definition the tests hold the library to, bit for bit).  Attention is the
+ * operation above over those values; the output tolerance is the same.
+ *   q, k_new, v_new  DEVICE bf16 as in cp_attention_step (k_new / v_new may be NULL: the caller wrote codes
+ *                    and scales itself); kv_cache8 DEVICE uint8; kv_scale DEVICE float32; out DEVICE bf16.
+ * As in cp_attention_step the unused slots of each request's last page are cleared (code 0, scale 1).
+ * Decodes (<= 8 rows per KV head) stream the fp8 pages straight into fp8 tensor-core MMAs; requests with a
+ * prefill chunk have their pages dequantised (exactly) into the library's bf16 scratch pool first and run the
+ * bf16 tile path over it.  Errors: CP_ESTATE (context not created with CP_KV_E4M3, no batch), CP_EINVAL, CP_ECUDA;
+ * cp_build_batch returns CP_ECAPACITY when the batch needs more scratch pages than max_scratch_pages. */
+int cp_attention_step_fp8(cp_ctx* ctx, int32_t layer, const void* q, const void* k_new, const void* v_new,
+                          void* kv_cache8, void* kv_scale, void* out, void* cuda_stream);
 
 /* H6: drain the ring of timed steps, oldest first, into rows (HOST, capacity cap);
  * *n_out receives the count.  Waits for the newest recorded step to finish.  The memory

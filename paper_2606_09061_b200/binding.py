@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libcp.so")
 
 CP_OK, CP_EINVAL, CP_ECAPACITY, CP_ECUDA, CP_ESTATE = 0, -1, -2, -3, -4
 CP_REQ_PREFILL = 1
+CP_KV_BF16, CP_KV_E4M3 = 0, 1
 CP_MODE_TOKEN_BUDGET, CP_MODE_LPRS = 0, 1
 CP_PRED_LINEAR, CP_PRED_MLP = 0, 1
 CP_NUM_RAW_FEATURES = 11
@@ -27,7 +28,7 @@ EXPORTS = [
     "cp_sched_destroy", "cp_sched_add_request", "cp_sched_next", "cp_sched_commit",
     "cp_sched_next_arrival", "cp_sched_has_work", "cp_sched_get_stats",
     "cp_sched_request_times", "cp_sched_predict", "cp_sched_select_chunk",
-    "cp_enable_rope", "cp_attention_step_rope",
+    "cp_enable_rope", "cp_attention_step_rope", "cp_attention_step_fp8",
 ]
 
 
@@ -36,7 +37,8 @@ class cp_config(C.Structure):
                 ("block_size", C.c_int32), ("num_layers", C.c_int32), ("num_blocks", C.c_int64),
                 ("sm_scale", C.c_float), ("max_tokens", C.c_int32), ("max_reqs", C.c_int32),
                 ("max_total_pages", C.c_int64), ("max_partial_rows", C.c_int64),
-                ("device", C.c_int32), ("kernel_variant", C.c_int32)]
+                ("device", C.c_int32), ("kernel_variant", C.c_int32), ("kv_dtype", C.c_int32),
+                ("reserved", C.c_int32), ("max_scratch_pages", C.c_int64)]
 
 
 class cp_req_desc(C.Structure):
@@ -104,6 +106,7 @@ def load(path: Optional[str] = None):
     lib.cp_build_batch.argtypes = [C.c_void_p, C.POINTER(cp_req_desc), C.c_int32, C.c_void_p]
     lib.cp_attention_step.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     lib.cp_attention_step_rope.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
+    lib.cp_attention_step_fp8.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 7
     lib.cp_enable_rope.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     lib.cp_latency_table.argtypes = [C.c_void_p, C.POINTER(cp_latency_row), C.c_int32,
                                      C.POINTER(C.c_int32)]
@@ -168,7 +171,8 @@ class Context:
 
     def __init__(self, num_q_heads, num_kv_heads, head_dim, num_blocks, block_size=16,
                  num_layers=1, sm_scale=None, max_tokens=8192, max_reqs=1024,
-                 max_total_pages=None, max_partial_rows=0, device=0, kernel_variant=0):
+                 max_total_pages=None, max_partial_rows=0, device=0, kernel_variant=0, kv_dtype=0,
+                 max_scratch_pages=0):
         self.lib = load()
         if sm_scale is None:
             sm_scale = float(np.float32(1.0) / np.sqrt(np.float32(head_dim)))
@@ -176,7 +180,7 @@ class Context:
             max_total_pages = int(num_blocks)
         self.cfg = cp_config(num_q_heads, num_kv_heads, head_dim, block_size, num_layers,
                              num_blocks, sm_scale, max_tokens, max_reqs, max_total_pages,
-                             max_partial_rows, device, kernel_variant)
+                             max_partial_rows, device, kernel_variant, kv_dtype, 0, max_scratch_pages)
         self.handle = C.c_void_p()
         _check(self.lib.cp_create(C.byref(self.cfg), C.byref(self.handle)))
         self._keep = None
@@ -201,6 +205,10 @@ class Context:
     def cp_attention_step_rope(self, layer, q, k_new, v_new, kv_cache, out, stream=None):
         _check(self.lib.cp_attention_step_rope(self.handle, layer, _ptr(q), _ptr(k_new), _ptr(v_new),
                                                _ptr(kv_cache), _ptr(out), _ptr(stream)))
+
+    def cp_attention_step_fp8(self, layer, q, k_new, v_new, kv_cache8, kv_scale, out, stream=None):
+        _check(self.lib.cp_attention_step_fp8(self.handle, layer, _ptr(q), _ptr(k_new), _ptr(v_new),
+                                              _ptr(kv_cache8), _ptr(kv_scale), _ptr(out), _ptr(stream)))
 
     def cp_latency_table(self, cap=4096) -> List[cp_latency_row]:
         rows = (cp_latency_row * cap)()

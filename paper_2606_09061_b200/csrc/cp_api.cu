@@ -114,6 +114,12 @@ struct cp_ctx {
     uint32_t mark_epoch = 0;
 #endif
 
+    // fp8 pools (cfg.kv_dtype == CP_KV_E4M3): the bf16 scratch pool of the requests with a prefill chunk
+    bool kv8 = false;
+    __nv_bfloat16* d_scratch = nullptr;
+    int64_t max_scratch_pages = 0;
+    int32_t scratch_pages = 0;         // in use by the current batch
+    std::vector<int32_t> scratch_base, scratch_req;
     // tensor-core path: one TMA descriptor per KV pool pointer (one per layer), encoded once
     std::vector<std::pair<const void*, CUtensorMap>> tmaps;
     void* encode_fn = nullptr;
@@ -128,6 +134,9 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     if (!(G == 1 || G == 2 || G == 4 || G == 8 || G == 16)) { cp_set_error("cp_create: G = Hq/Hkv must be in {1,2,4,8,16}"); return CP_EINVAL; }
     if (!(D == 64 || D == 128)) { cp_set_error("cp_create: head_dim must be 64 or 128"); return CP_EINVAL; }
     if (cfg->block_size != 16) { cp_set_error("cp_create: block_size must be 16"); return CP_EINVAL; }
+    if (cfg->kv_dtype != CP_KV_BF16 && cfg->kv_dtype != CP_KV_E4M3) { cp_set_error("cp_create: kv_dtype must be CP_KV_BF16 or CP_KV_E4M3"); return CP_EINVAL; }
+    if (cfg->kv_dtype == CP_KV_E4M3 && (D != 128 || G > 16 || cfg->kernel_variant != 0)) { cp_set_error("cp_create: e4m3 pools need head_dim 128"); return CP_EINVAL; }
+    if (cfg->reserved != 0 || cfg->max_scratch_pages < 0) { cp_set_error("cp_create: reserved must be 0, max_scratch_pages >= 0"); return CP_EINVAL; }
     if (cfg->num_blocks < 1 || cfg->max_tokens < 1 || cfg->max_reqs < 1 || cfg->max_total_pages < 1 ||
         cfg->num_layers < 1) { cp_set_error("cp_create: limits must be positive"); return CP_EINVAL; }
     if ((int64_t)cfg->num_blocks * 2 * Hkv >= (int64_t)1 << 31) { cp_set_error("cp_create: pool too large for 32-bit slab index"); return CP_EINVAL; }
@@ -160,6 +169,9 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     cap += align_up(sizeof(int32_t) * cfg->max_reqs, 16) * 2;            // q_len, ctx_off
     cap += align_up(sizeof(int32_t) * (size_t)cfg->max_total_pages, 16);
     cap += align_up(sizeof(int32_t) * (size_t)cfg->max_tokens, 16);      // tok_req
+    c->kv8 = cfg->kv_dtype == CP_KV_E4M3;
+    c->max_scratch_pages = c->kv8 ? (cfg->max_scratch_pages > 0 ? cfg->max_scratch_pages : cfg->max_total_pages) : 0;
+    if (c->kv8) cap += align_up(sizeof(int32_t) * cfg->max_reqs, 16) + align_up(sizeof(int32_t) * (size_t)c->max_scratch_pages, 16);
     cap += align_up(sizeof(WorkItem) * c->max_items, 16);
     cap += align_up(sizeof(CombineItem) * c->max_combine, 16);
     c->meta_cap = cap;
@@ -170,6 +182,7 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     chk(cudaMalloc(&c->d_part_o, sizeof(float) * (size_t)c->max_partial_rows * D));
     chk(cudaMalloc(&c->d_part_ml, sizeof(float2) * (size_t)c->max_partial_rows));
     chk(cudaMalloc(&c->d_counter, sizeof(int32_t) * 4));
+    if (c->kv8) chk(cudaMalloc(&c->d_scratch, sizeof(__nv_bfloat16) * (size_t)c->max_scratch_pages * 2 * Hkv * cfg->block_size * D));
     chk(cudaMemset(c->d_counter, 0, sizeof(int32_t) * 4));
     for (int i = 0; i < kMetaRing; ++i) {
         chk(cudaMallocHost(&c->h_stage[i], cap));
@@ -207,6 +220,7 @@ extern "C" int cp_destroy(cp_ctx* c) {
     cudaFree(c->d_part_o);
     cudaFree(c->d_part_ml);
     cudaFree(c->d_counter);
+    cudaFree(c->d_scratch);
     cudaFree(c->d_inv_freq);
     cudaFree(c->d_rope_cs);
     cudaFree(c->d_q_rot);
@@ -289,13 +303,15 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
         const double bytes = 2.0 * alg_keys * sh.Hkv * sh.D * 2 + 2.0 * (double)T * sh.Hq * sh.D * 2;
         tensor_bound = c->use_tc && flops / 2.25e15 > bytes / 8e12;
     }
+    if (c->kv8) tensor_bound = false;                    // fp8 pools: always the dual-lane instantiation
     const int TQ = c->tq;                                // tokens per tile-kind item
+    const int swap_rows = c->kv8 ? 8 : 16;               // rows of a swap-kind item (fp8: hi / lo codes share the 16 B rows)
     for (int j = 0; j < n_reqs; ++j) {
         const cp_req_desc& r = reqs[j];
         for (int q0 = 0; q0 < r.q_len; q0 += TQ) {
             const int qt = std::min(TQ, r.q_len - q0);
             const int64_t lim = (int64_t)r.ctx_off + q0 + qt;
-            const int kind = (c->use_tc && qt * G <= 16 && sh.D == 128) ? kKindSwap : kKindTile;
+            const int kind = (c->use_tc && qt * G <= swap_rows && sh.D == 128) ? kKindSwap : kKindTile;
             total_tiles[kind] += (lim + kKeyTile - 1) / kKeyTile * sh.Hkv;
         }
     }
@@ -336,7 +352,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
                 const int q0 = qi * TQ, qt = std::min(TQ, r.q_len - q0), rows = qt * G;
                 const int lim = r.ctx_off + q0 + qt;                 // causal limit of the last row
                 const int n_tiles = (lim + kKeyTile - 1) / kKeyTile;
-                const int chunk_tiles = chunk_of[(c->use_tc && rows <= 16 && sh.D == 128) ? kKindSwap : kKindTile];
+                const int chunk_tiles = chunk_of[(c->use_tc && rows <= swap_rows && sh.D == 128) ? kKindSwap : kKindTile];
                 const int n_splits = (n_tiles + chunk_tiles - 1) / chunk_tiles;
                 c->plan[2 * qi] = n_splits;
                 c->plan[2 * qi + 1] = (n_tiles + n_splits - 1) / n_splits;
@@ -364,7 +380,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
                         if (s >= c->plan[2 * qi]) continue;
                         const int q0 = qi * TQ, qt = std::min(TQ, r.q_len - q0), rows = qt * G;
                         const int lim = r.ctx_off + q0 + qt, tps = c->plan[2 * qi + 1];
-                        const int kind = (c->use_tc && rows <= 16 && sh.D == 128) ? kKindSwap : kKindTile;
+                        const int kind = (c->use_tc && rows <= swap_rows && sh.D == 128) ? kKindSwap : kKindTile;
                         const int32_t prow = c->plan_prow[(size_t)qi * sh.Hkv + g];
                         if (c->items.size() >= c->max_items) { overflow = true; break; }
                         c->items.push_back(WorkItem{j, g, q0, qt, s * tps * kKeyTile, std::min(lim, (s + 1) * tps * kKeyTile),
@@ -415,6 +431,29 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     const size_t o_tr = place(sizeof(int32_t) * (size_t)T);
     const size_t o_wk = place(sizeof(WorkItem) * n_items);
     const size_t o_cb = place(sizeof(CombineItem) * c->combines.size());
+    // fp8 pools: requests with a tile-kind item get their pages dequantised into the scratch pool, contiguously
+    size_t o_sb = 0, o_sr = 0;
+    if (c->kv8) {
+        c->scratch_base.assign((size_t)n_reqs, -1);
+        c->scratch_req.clear();
+        for (const WorkItem& w : c->items)
+            if (w.kind == kKindTile && c->scratch_base[w.req] < 0) c->scratch_base[w.req] = 0;      // mark
+        int64_t used = 0;
+        for (int j = 0; j < n_reqs; ++j) {
+            if (c->scratch_base[j] < 0) continue;
+            const int used_pages = (int)(((int64_t)reqs[j].ctx_off + reqs[j].q_len + B - 1) / B);
+            if (used + used_pages > c->max_scratch_pages) {
+                cp_set_error("cp_build_batch: the prefill chunks of this batch need more than max_scratch_pages = %lld scratch pages",
+                             (long long)c->max_scratch_pages);
+                return CP_ECAPACITY;
+            }
+            c->scratch_base[j] = (int32_t)used;
+            c->scratch_req.insert(c->scratch_req.end(), (size_t)used_pages, j);
+            used += used_pages;
+        }
+        o_sb = place(sizeof(int32_t) * n_reqs);
+        o_sr = place(sizeof(int32_t) * c->scratch_req.size());
+    }
     if (off > c->meta_cap) { cp_set_error("cp_build_batch: metadata %zu B > capacity %zu B", off, c->meta_cap); return CP_ECAPACITY; }
     int32_t* cu = reinterpret_cast<int32_t*>(h + o_cu);
     int32_t* ql = reinterpret_cast<int32_t*>(h + o_ql);
@@ -441,6 +480,11 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
         c->combine_rows = rows;
     }
     std::memcpy(h + o_cb, c->combines.data(), sizeof(CombineItem) * c->combines.size());
+    if (c->kv8) {
+        std::memcpy(h + o_sb, c->scratch_base.data(), sizeof(int32_t) * n_reqs);
+        std::memcpy(h + o_sr, c->scratch_req.data(), sizeof(int32_t) * c->scratch_req.size());
+        c->scratch_pages = (int32_t)c->scratch_req.size();
+    }
 
     // the copy runs on the library's own stream, next to the previous batch's steps; it waits only for the
     // steps that read this device slot kMetaRing batches ago, and the caller's stream waits for the copy
@@ -462,6 +506,8 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     m.tok_req = reinterpret_cast<const int32_t*>(d_meta + o_tr);
     m.work = reinterpret_cast<const WorkItem*>(d_meta + o_wk);
     m.combine = reinterpret_cast<const CombineItem*>(d_meta + o_cb);
+    m.scratch_base = c->kv8 ? reinterpret_cast<const int32_t*>(d_meta + o_sb) : nullptr;
+    m.scratch_req = c->kv8 ? reinterpret_cast<const int32_t*>(d_meta + o_sr) : nullptr;
     m.n_reqs = n_reqs;
     m.n_tokens = (int32_t)T;
     m.n_work = (int32_t)n_items;
@@ -544,9 +590,12 @@ typedef CUresult (*cuTensorMapEncodeTiled_t)(CUtensorMap*, CUtensorMapDataType, 
                                              CUtensorMapFloatOOBfill);
 
 // TMA descriptor of one layer's KV pool (slab = (block, K|V, kv head)), 128-byte swizzle.
-static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out) {
+// kind 0: a bf16 pool of n_pages pages; kind 1: an e4m3 pool (one box = the 16 x 128 B codes of a slab).
+static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out, int kind = 0, int64_t n_pages = 0) {
+    if (n_pages == 0) n_pages = c->cfg.num_blocks;
+    const void* key = static_cast<const uint8_t*>(kv_cache) + kind;     // pools are 16-byte aligned: the low bit tags the kind
     for (auto& e : c->tmaps)
-        if (e.first == kv_cache) { *out = &e.second; return CP_OK; }
+        if (e.first == key) { *out = &e.second; return CP_OK; }
     if (!c->encode_fn) {
         cudaDriverEntryPointQueryResult qres;
         CP_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &c->encode_fn, cudaEnableDefault, &qres));
@@ -557,6 +606,21 @@ static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out) {
     }
     const Shape& sh = c->shape;
     CUtensorMap m;
+    if (kind == 1) {
+        // e4m3 pool: 3-D {D bytes, 16 slots, slabs}; a box = one slab = 16 rows of 128 B = two 8-row swizzle groups
+        const cuuint64_t dims[3] = {(cuuint64_t)sh.D, 16, (cuuint64_t)n_pages * 2 * sh.Hkv};
+        const cuuint64_t strides[2] = {(cuuint64_t)sh.D, (cuuint64_t)sh.D * 16};
+        const cuuint32_t box[3] = {(cuuint32_t)sh.D, 16, 1};
+        const cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = reinterpret_cast<cuTensorMapEncodeTiled_t>(c->encode_fn)(
+            &m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, kv_cache, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { cp_set_error("cuTensorMapEncodeTiled (e4m3 pool) failed: %d", (int)r); return CP_ECUDA; }
+        if (c->tmaps.size() >= 256) c->tmaps.clear();
+        c->tmaps.emplace_back(key, m);
+        *out = &c->tmaps.back().second;
+        return CP_OK;
+    }
     // 5-D view of the pool so that ONE box = one whole (block, K|V, head) slab of 16 tokens x D:
     //   d0 64 elements (one 128-byte half-row)     d1 8 tokens of a row group (stride D*2)
     //   d2 D/64 halves of a row (stride 128 B)     d3 2 row groups (stride 8*D*2)
@@ -564,7 +628,7 @@ static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out) {
     // The box lands in smem as [row group][half][8 rows][128 B]: 8-row groups of each half are
     // D/64 KiB apart for the whole 128-key tile, which is a legal UMMA SBO (see cp_kernels_dl.cuh).
     const cuuint64_t rowb = (cuuint64_t)sh.D * 2;
-    const cuuint64_t dims[5] = {64, 8, (cuuint64_t)sh.D / 64, 2, (cuuint64_t)c->cfg.num_blocks * 2 * sh.Hkv};
+    const cuuint64_t dims[5] = {64, 8, (cuuint64_t)sh.D / 64, 2, (cuuint64_t)n_pages * 2 * sh.Hkv};
     const cuuint64_t strides[4] = {rowb, 128, 8 * rowb, 16 * rowb};
     const cuuint32_t box[5] = {64, 8, (cuuint32_t)sh.D / 64, 2, 1};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
@@ -573,33 +637,45 @@ static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out) {
         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { cp_set_error("cuTensorMapEncodeTiled failed: %d", (int)r); return CP_ECUDA; }
     if (c->tmaps.size() >= 256) c->tmaps.clear();
-    c->tmaps.emplace_back(kv_cache, m);
+    c->tmaps.emplace_back(key, m);
     *out = &c->tmaps.back().second;
     return CP_OK;
 }
 
+// kv_scale != nullptr: kv_cache is an e4m3 pool (D = 128), chunk tiles read the library's bf16 scratch pool
 template <int D>
-static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_bfloat16* out, cudaStream_t stream,
-                       int* launches) {
+static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const float* kv_scale, __nv_bfloat16* out,
+                       cudaStream_t stream, int* launches) {
     const BatchMeta& m = c->meta;
     const CUtensorMap* tmap = nullptr;
-    int rc = get_tmap(c, kv_cache, &tmap);
+    const CUtensorMap* tmap8 = nullptr;
+    int rc = kv_scale ? get_tmap(c, c->d_scratch, &tmap, 0, c->max_scratch_pages) : get_tmap(c, kv_cache, &tmap);
     if (rc != CP_OK) return rc;
+    // (get_tmap may clear its cache when it grows: take the second descriptor's copy before it could move)
+    const CUtensorMap tmap_copy = *tmap;
+    if (kv_scale) { rc = get_tmap(c, kv_cache, &tmap8, 1); if (rc != CP_OK) return rc; }
+    else tmap8 = &tmap_copy;
     if (!c->tc_attr_set) {
-        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D, false>::kTotal));
-        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D, true>::kTotal));
+        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D, false>::kTotal));
+        CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D, true>::kTotal));
+        if constexpr (D == 128)
+            CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<128, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<128, false>::kTotal));
         c->tc_attr_set = true;
     }
     if (m.n_work > 0) {
         const int grid = std::min(c->n_sm, m.n_work);
-        dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter};
+        dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, kv_scale};
+        if (kv_scale) {
+            if constexpr (D == 128)
+                CP_CUDA(launch_pdl(dl::attn_dl_kernel<128, false, false, true>, dim3(grid), dim3(dl::kThreads), dl::Layout<128, false>::kTotal, stream, p, tmap_copy, *tmap8));
+        } else
         // Two instantiations of the one kernel, chosen per batch by the SURVEY.md 8(d) roofline formulas: HBM-bound
         // batches run chunk tiles and decode streams side by side (dual lane); tensor-bound batches put both softmax
         // warpgroups on every chunk tile (SPLIT) and move a quarter of the exponentials to the FMA pipe.
         if (c->tensor_bound)
-            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, true, true>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, true>::kTotal, stream, p, *tmap));
+            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, true, true, false>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, true>::kTotal, stream, p, tmap_copy, *tmap8));
         else
-            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, false, false>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, false>::kTotal, stream, p, *tmap));
+            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, false, false, false>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, false>::kTotal, stream, p, tmap_copy, *tmap8));
         CP_CUDA(cudaGetLastError());
         ++*launches;
         c->info.grid_attn = grid;
@@ -613,16 +689,20 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, __nv_b
     return CP_OK;
 }
 
-static int launch_tc(cp_ctx* c, const __nv_bfloat16* q, __nv_bfloat16* kv_cache, __nv_bfloat16* out,
+static int launch_tc(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const float* kv_scale, __nv_bfloat16* out,
                      cudaStream_t stream, int* launches) {
-    return c->shape.D == 128 ? launch_tc_d<128>(c, q, kv_cache, out, stream, launches)
-                             : launch_tc_d<64>(c, q, kv_cache, out, stream, launches);
+    return c->shape.D == 128 ? launch_tc_d<128>(c, q, kv_cache, kv_scale, out, stream, launches)
+                             : launch_tc_d<64>(c, q, kv_cache, kv_scale, out, stream, launches);
 }
 
 static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new, const void* v_new,
-                          void* kv_cache, void* out, void* stream_, bool rope) {
+                          void* kv_cache, void* out, void* stream_, bool rope, void* kv_scale = nullptr) {
     if (!c) return CP_EINVAL;
     if (!c->have_batch) { cp_set_error("cp_attention_step: no batch built"); return CP_ESTATE; }
+    if (c->kv8 != (kv_scale != nullptr)) {
+        cp_set_error(c->kv8 ? "this context drives an e4m3 pool: use cp_attention_step_fp8" : "cp_attention_step_fp8: the context was not created with CP_KV_E4M3");
+        return CP_ESTATE;
+    }
     if (rope) {
         if (!c->d_rope_cs) { cp_set_error("cp_attention_step_rope: cp_enable_rope was not called"); return CP_ESTATE; }
         if (c->rope_table_iter != c->iter) {
@@ -659,6 +739,25 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
             CP_CUDA(cudaGetLastError());
             ++launches;
             q = c->d_q_rot;
+        } else if (kv_scale) {
+            // quantise the new rows into the e4m3 pages (and clear the page tails), then dequantise the pages of
+            // the requests with a prefill chunk into the bf16 scratch pool
+            const Shape& sh = c->shape;
+            const int64_t total = std::max<int64_t>(k_new ? (int64_t)m.n_tokens * sh.Hkv * 2 * 16 : 0,
+                                                    (int64_t)m.n_reqs * 2 * sh.Hkv * (sh.B - 1) * (sh.D / 16));
+            const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 8);
+            kv_append_q8_kernel<<<grid, 256, 0, stream>>>(m, sh, static_cast<const uint4*>(k_new), static_cast<const uint4*>(v_new),
+                                                          static_cast<uint8_t*>(kv_cache), static_cast<float*>(kv_scale));
+            CP_CUDA(cudaGetLastError());
+            ++launches;
+            if (c->scratch_pages > 0) {
+                const int64_t units = (int64_t)c->scratch_pages * 2 * sh.Hkv * sh.B * (sh.D / 16);
+                const int g2 = (int)std::min<int64_t>((units + 255) / 256, (int64_t)c->n_sm * 16);
+                kv8_dequant_kernel<<<g2, 256, 0, stream>>>(m, sh, static_cast<const uint8_t*>(kv_cache), static_cast<const float*>(kv_scale),
+                                                           c->d_scratch, c->scratch_pages);
+                CP_CUDA(cudaGetLastError());
+                ++launches;
+            }
         } else {
             // k_new == NULL (the caller wrote the pages): the kernel only zeroes the stale page tails
             const int64_t total = std::max<int64_t>(k_new ? (int64_t)m.n_tokens * c->shape.Hkv * (c->shape.D / 8) * 2 : 0,
@@ -684,7 +783,7 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
         } else
 #endif
         {
-            rc = launch_tc(c, static_cast<const __nv_bfloat16*>(q), static_cast<__nv_bfloat16*>(kv_cache),
+            rc = launch_tc(c, static_cast<const __nv_bfloat16*>(q), kv_cache, static_cast<const float*>(kv_scale),
                            static_cast<__nv_bfloat16*>(out), stream, &launches);
         }
         if (rc != CP_OK) return rc;
@@ -707,6 +806,12 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
 extern "C" int cp_attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new,
                                  const void* v_new, void* kv_cache, void* out, void* stream) {
     return attention_step(c, layer, q, k_new, v_new, kv_cache, out, stream, false);
+}
+
+extern "C" int cp_attention_step_fp8(cp_ctx* c, int32_t layer, const void* q, const void* k_new, const void* v_new,
+                                     void* kv_cache8, void* kv_scale, void* out, void* stream) {
+    if (!kv_scale || (reinterpret_cast<uintptr_t>(kv_scale) & 15)) { cp_set_error("cp_attention_step_fp8: kv_scale must be a 16-byte aligned device pointer"); return CP_EINVAL; }
+    return attention_step(c, layer, q, k_new, v_new, kv_cache8, out, stream, false, kv_scale);
 }
 
 extern "C" int cp_attention_step_rope(cp_ctx* c, int32_t layer, const void* q, const void* k_new,

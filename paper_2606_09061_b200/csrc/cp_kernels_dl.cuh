@@ -56,6 +56,8 @@ namespace dl {
 constexpr int kThreads = 512;
 constexpr int kStagesT = 3, kStagesS = 3, kMaxStages = 6;
 constexpr int kStagesSplit = 6, kProdSplit = 5;  // SPLIT mode: one ring, all five producer warps
+constexpr int kStagesS8 = 6;                     // fp8 pools: lane S's ring is six 16 KiB slots (same bytes in flight)
+constexpr uint32_t kSlot8Bytes = 16384, kPage8Bytes = 2048;   // a 128-key fp8 tile (D = 128); a 16-token page slab
 constexpr int kProdT = 3, kProdS = 2;         // TMA producer warps per lane (kProdT + kProdS + 3 MMA warps = 8 warps)
 // a producer waiting for slot reuse may be at most one phase behind only if kProd <= kStages
 static_assert(kProdT <= kStagesT && kProdS <= kStagesS && kProdT + kProdS == 5, "producer / stage configuration");
@@ -116,6 +118,7 @@ struct LaneState {              // one per lane, in the misc region
     WorkItem items[kItemRing];  // published by the lane's producer; kind < 0 = no more work
     float cmax[2][4][16];       // swap kind: per-warp column maxima, double buffered
     float lsum[4][16];          // swap kind: per-warp column sums at the end of an item
+    float qs[8];                // fp8 swap kind: per-row scale of the quantised Q^T
 };
 
 struct Misc {
@@ -132,6 +135,7 @@ struct Params {
     float* part_o;
     float2* part_ml;
     int32_t* counters;          // [0] next tile item, [1] next swap item, [2] finished CTAs
+    const float* kv_scale;      // fp8 pools: [block][K|V][kv head][slot] power-of-two row scales, else unused
 };
 
 // element e of a half-tile row: MUFU or FMA-pipe exponential (e is a constant after unrolling)
@@ -181,11 +185,16 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
 // instruction footprint has to stay inside the 32 KB L1.5 instruction cache of the SM -- with one copy
 // per lane (and the other per-lane duplicates) it was 39 KB in a mixed batch and the tile softmax spent
 // 40-50 % of its issue slots waiting for instruction fetch (ncu: stall_no_inst; 4 % in a chunk-only batch).
-template <int D, bool SPLIT>
-__device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tmap, uint8_t* smem, Misc* misc, int lane, int warp) {
+// fp8 pools (KV8): swap-kind items stream the e4m3 pages themselves (tmap8: one 2 KiB box per page, 16 KiB per
+// 128-key tile; lane S's ring is six such slots, lane T's slots keep their 32 KiB stride); tile-kind items read
+// the request's dequantised pages from the library's bf16 scratch pool (tmap), where they are contiguous from
+// scratch_base[req] -- no block table.
+template <int D, bool SPLIT, bool KV8>
+__device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tmap, const CUtensorMap* tmap8, uint8_t* smem, Misc* misc, int lane, int warp) {
     using L = Layout<D, SPLIT>;
     static_assert(kStagesT == kStagesS, "the shared producer code assumes one ring depth");
-    constexpr int kStages = L::kStages;
+    const int kStages = (KV8 && warp >= kProdT) ? kStagesS8 : L::kStages;
+    const uint32_t slot_bytes = (KV8 && warp >= kProdT) ? kSlot8Bytes : L::kSlotBytes;
     const int LANE = SPLIT ? 0 : (warp < kProdT ? 0 : 1);
     const int pw = LANE == 0 ? warp : warp - kProdT;
     const int kProd = SPLIT ? kProdSplit : (LANE == 0 ? kProdT : kProdS);
@@ -229,10 +238,14 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
         const int n_tiles = (kv_end - kv_begin + kKeyTile - 1) / kKeyTile;
         const int32_t* bt = p.meta.block_table + p.meta.bt_off[req] + (kv_begin >> 4);
         const int n_pages_item = (kv_end - kv_begin + 15) >> 4;
+        const bool fp8_item = KV8 && __shfl_sync(0xffffffffu, w, 7) == kKindSwap;
+        const bool scratch = KV8 && !fp8_item;
+        const int sbase = scratch ? p.meta.scratch_base[req] + (kv_begin >> 4) : 0;
+        auto page_id = [&](int i) { return scratch ? sbase + i : bt[i]; };
         // page-id windows of 32 pages (4 tiles), one id per lane: cur = window cur_w, nxt = the next
         int cur_w = 0;
-        int cur = lane < n_pages_item ? bt[lane] : 0;
-        int nxt = 32 + lane < n_pages_item ? bt[32 + lane] : 0;
+        int cur = lane < n_pages_item ? page_id(lane) : 0;
+        int nxt = 32 + lane < n_pages_item ? page_id(32 + lane) : 0;
         // load number ld = ld_base + i (global over the whole kernel) belongs to producer ld % kProd, so a
         // producer's previous load is always ld - kProd: with kProd <= kStages the slot it waits for is at
         // most one phase behind and the parity wait cannot alias
@@ -246,21 +259,22 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
                 cur = nxt;
                 ++cur_w;
                 const int pi = (cur_w + 1) * 32 + lane;
-                nxt = pi < n_pages_item ? bt[pi] : 0;
+                nxt = pi < n_pages_item ? page_id(pi) : 0;
             }
             const int n_pages = min(8, n_pages_item - tile * 8);          // 1..8
             const uint32_t ld = ld_base + i;
             const uint32_t slot = ld % kStages;
             ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1);
             const bool leader = ptx::elect_one();
-            if (leader) ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * 16u * D * 2u);
-            uint8_t* dst = kv_base + slot * L::kSlotBytes;
+            if (leader) ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * (fp8_item ? kPage8Bytes : 16u * D * 2u));
+            uint8_t* dst = kv_base + slot * slot_bytes;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 const int pg = __shfl_sync(0xffffffffu, cur, (tile & 3) * 8 + j);
                 if (j < n_pages) {
                     const int slab = (pg * 2 + is_v) * p.sh.Hkv + kv_head;
-                    if (leader) ptx::tma_load_5d(dst + j * L::kPageBytes, tmap, &ls->kv_full[slot], 0, 0, 0, 0, slab);
+                    if (KV8 && fp8_item) { if (leader) ptx::tma_load_3d(dst + j * kPage8Bytes, tmap8, &ls->kv_full[slot], 0, 0, slab); }
+                    else if (leader) ptx::tma_load_5d(dst + j * L::kPageBytes, tmap, &ls->kv_full[slot], 0, 0, 0, 0, slab);
                 }
             }
             __syncwarp();
@@ -417,7 +431,74 @@ __device__ __forceinline__ void mma_split_item(const WorkItem& it, uint32_t smem
     ld_base += 2 * n_tiles;
 }
 
-template <int D, int LANE, int ROLE, bool SPLIT>
+// fp8 pools, swap kind (<= 8 rows, D = 128): the e4m3 pages feed kind::f8f6f4 MMAs directly (K = 32 per instruction).
+// Both operands must be 8-bit, so Q^T and P^T come as e4m3 too, each value split x = hi + lo / 16 into two codes
+// stacked along N (rows 0..7 = hi, 8..15 = lo of the 16-row B operand: N = 16 as in the bf16 kind) -- ~2^-8 relative,
+// what bf16 gives; the softmax adds the two column groups after tcgen05.ld.
+//   S^T[128 keys x 16] = K[128 x D] Q8^T      (A = K tile, K-major, 4 K-steps of 32 d)
+//   O^T[128 d x 16]   += V^T[D x 128] P8^T    (A = V tile MN-major, 4 K-steps of 32 keys; B = P8^T, K-major along keys)
+// Same barriers and tile order as the bf16 swap kind.  Lane S's ring: six 16 KiB slots; lane T's: 32 KiB stride.
+template <int D, int LANE>
+__device__ __forceinline__ void mma_swap8_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
+                                               uint32_t& ld_base, uint32_t& gt, uint32_t& gp, uint32_t& ic) {
+    using L = Layout<D, false>;
+    constexpr int kStages = LANE == 0 ? kStagesT : kStagesS8;
+    constexpr uint32_t kStride = LANE == 0 ? L::kSlotBytes : kSlot8Bytes;
+    const int n_tiles = (__shfl_sync(0xffffffffu, it.kv_end - it.kv_begin, 0) + kKeyTile - 1) / kKeyTile;
+    const uint32_t small = smem_base + L::kOffSmall[LANE], kv_base = smem_base + L::kOffKv[LANE];
+    const uint32_t idesc_qk = ptx::umma_idesc_e4m3(128, 16, false, false);
+    const uint32_t idesc_pv = ptx::umma_idesc_e4m3(128, 16, true, false);
+    const uint32_t g0 = gt;
+    ptx::mbar_wait(&ls->q_full[1], ic & 1);
+    ptx::tc_fence_after();
+    ++ic;
+    auto issue_qk = [&](int t) {
+        const uint32_t ld = ld_base + (t == 0 ? 0 : 2 * t - 1);
+        const uint32_t slot = ld % kStages, buf = (g0 + t) & 1;
+        ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+        ptx::tc_fence_after();
+        if (ptx::elect_one()) {
+            const uint64_t k_desc0 = ptx::umma_desc_sw128(kv_base + slot * kStride, 16, 1024);     // rows of 128 B, 8-row groups 1 KB apart
+            const uint64_t q_desc0 = ptx::umma_desc_sw128(small, 16, 1024);
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks)
+                ptx::umma_ss_f8(tmem + col_s(LANE, buf), ptx::umma_desc_advance(k_desc0, ks * 32), ptx::umma_desc_advance(q_desc0, ks * 32),
+                                idesc_qk, ks > 0);
+            ptx::umma_commit(&ls->kv_empty[slot]);
+            ptx::umma_commit(&ls->s_full[buf]);
+        }
+        __syncwarp();
+    };
+    auto issue_pv = [&](int t) {
+        const uint32_t ld = ld_base + (t == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * t + 2);
+        const uint32_t slot = ld % kStages, buf = (g0 + t) & 1;
+        ptx::mbar_wait(&ls->p_full[1][gp & 1], (gp >> 1) & 1);
+        ++gp;
+        ptx::mbar_wait(&ls->kv_full[slot], (ld / kStages) & 1);
+        ptx::tc_fence_after();
+        if (ptx::elect_one()) {
+            // V (MN-major, 8-bit): a key row is 128 B = all 128 d; 32 keys = 4 row groups, SBO = 1 KB apart
+            const uint64_t v_desc0 = ptx::umma_desc_sw128(kv_base + slot * kStride, 1024, 1024);
+            const uint64_t p_desc0 = ptx::umma_desc_sw128(small + 4096 + buf * 4096, 16, 1024);     // P8^T is double buffered
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks)
+                ptx::umma_ss_f8(tmem + col_o(LANE), ptx::umma_desc_advance(v_desc0, ks * 4096), ptx::umma_desc_advance(p_desc0, ks * 32),
+                                idesc_pv, t > 0 || ks > 0);
+            ptx::umma_commit(&ls->kv_empty[slot]);
+            ptx::umma_commit(&ls->pv_done[buf]);
+        }
+        __syncwarp();
+    };
+    issue_qk(0);
+    for (int t = 0; t < n_tiles; ++t) {
+        if (t + 1 < n_tiles) issue_qk(t + 1);
+        issue_pv(t);
+    }
+    gt += n_tiles;
+    ld_base += 2 * n_tiles;
+}
+
+template <int D, int LANE, int ROLE, bool SPLIT, bool KV8>
 __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base, LaneState* ls, uint32_t tmem,
                                          uint32_t& ld_base, uint32_t& gt, uint32_t& gp, uint32_t (&ic)[2], uint32_t& gpt) {
     using L = Layout<D, SPLIT>;
@@ -433,6 +514,10 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
     if (ROLE == 2) {                           // swap item on lane T: ROLE 1 issues it; stay in step
         gt += n_tiles;
         ld_base += 2 * n_tiles;
+        return;
+    }
+    if constexpr (KV8 && D == 128) {
+        mma_swap8_item<D, LANE>(it, smem_base, ls, tmem, ld_base, gt, gp, ic[1]);
         return;
     }
     const bool do_qk = all || ROLE == 1, do_pv = all || ROLE == 2;
@@ -522,7 +607,7 @@ __device__ __forceinline__ void mma_item(const WorkItem& it, uint32_t smem_base,
     ld_base += 2 * n_tiles;
 }
 
-template <int D, int LANE, int ROLE, bool SPLIT>
+template <int D, int LANE, int ROLE, bool SPLIT, bool KV8>
 __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lane) {
     LaneState* ls = &misc->lane[LANE];
     const uint32_t tmem = misc->tmem_base;
@@ -534,7 +619,7 @@ __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lan
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&ls->item_empty[islot]);
         if (it.kind < 0) break;
-        mma_item<D, LANE, ROLE, SPLIT>(it, smem_base, ls, tmem, ld_base, gt, gp, ic, gpt);
+        mma_item<D, LANE, ROLE, SPLIT, KV8>(it, smem_base, ls, tmem, ld_base, gt, gp, ic, gpt);
         ++item_cnt;
     }
 }
@@ -839,6 +924,214 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
 // row; columns in [R, RC) are computed as fully masked.  Straight-line code per column so the
 // independent chains interleave; the column max is one REDUX per column and warp.
 // ------------------------------------------------------------------------------------------
+// fp8 pools: softmax warps of the swap kind (R <= RC <= 8 rows, D = 128): thread <-> key, as in softmax_swap.
+// What differs (mma_swap8_item): Q^T and P^T are e4m3 operands, every value split into two codes x = hi + lo / 16
+// stacked along N, so a score is S^T[key][c] + S^T[key][8 + c] / 16; the row scales of the pages are per key,
+// i.e. per THREAD here: the K scale multiplies the thread's scores; the V scale goes into the weight
+// w = p * vs (as an exponent shift lv = log2 vs, so the running maximum normalises w, not p, and w stays in
+// (0, 2^8] whatever the scale), and the row sum takes w / vs = p back.  Q rows are scaled to amax 448 per row
+// (qs[c], folded into the score).  One lg2 per thread and tile; nothing per element beyond the bf16 kind.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t e4m3_of(float x) {             // round to nearest even, saturating
+    uint16_t r;
+    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(r) : "f"(0.f), "f"(x));
+    return r & 0xffu;
+}
+__device__ __forceinline__ float e4m3_value(uint32_t code) {
+    uint32_t h2;
+    asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"((uint16_t)code));
+    return __half2float(__ushort_as_half((unsigned short)(h2 & 0xffffu)));
+}
+
+template <int LANE, int RC>
+__device__ __forceinline__ void softmax_swap8(const WorkItem& it, const Params& p, uint8_t* small, LaneState* ls,
+                                              uint32_t tmem, uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base, int swarp) {
+    constexpr int D = 128;
+    const Shape& sh = p.sh;
+    const int G = sh.G;
+    const int gs = 31 - __clz(G);
+    const int R = it.q_tokens * G;                       // <= RC
+    const int n_tiles = (it.kv_end - it.kv_begin + kKeyTile - 1) / kKeyTile;
+    const int tok0 = p.meta.cu_q[it.req] + it.q_start;
+    const int ctx = p.meta.ctx_off[it.req];
+    const float scale = sh.sm_scale * 1.4426950408889634f;
+    const int lane = row & 31;
+    const int32_t* bt = p.meta.block_table + p.meta.bt_off[it.req];
+
+    // ---- Q8^T -> smem: B operand [16 rows][128 B], K-major, 128B swizzle: row c = hi codes of Q row c, row 8 + c = lo codes.
+    // 16 threads per Q row, 8 elements each; the row maximum by shuffles inside the half-warp.
+    for (int id = row; id < RC * 16; id += 128) {
+        const int r = id >> 4, c = id & 15;
+        float x[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = 0.f;
+        if (r < R) {
+            const int tok = tok0 + (r >> gs), head = it.kv_head * G + (r & (G - 1));
+            const uint4 v = *reinterpret_cast<const uint4*>(p.q + ((int64_t)tok * sh.Hq + head) * D + c * 8);
+            const __nv_bfloat162* h2 = reinterpret_cast<const __nv_bfloat162*>(&v);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { const float2 f = __bfloat1622float2(h2[j]); x[2 * j] = f.x; x[2 * j + 1] = f.y; }
+        }
+        float amax = 0.f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) amax = fmaxf(amax, fabsf(x[j]));
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+        const float qs = amax > 0.f ? amax * (1.f / 448.f) : 1.f;
+        const float inv = 1.f / qs;
+        uint32_t hi[2] = {0, 0}, lo[2] = {0, 0};
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const float y = x[j] * inv;
+            const uint32_t h = e4m3_of(y);
+            const uint32_t l = e4m3_of((y - e4m3_value(h)) * 16.f);
+            hi[j >> 2] |= h << ((j & 3) * 8);
+            lo[j >> 2] |= l << ((j & 3) * 8);
+        }
+        const uint32_t off = (((uint32_t)(c >> 1) ^ (uint32_t)(r & 7)) << 4) + (c & 1) * 8;      // (8 + r) & 7 == r & 7
+        *reinterpret_cast<uint2*>(small + r * 128 + off) = make_uint2(hi[0], hi[1]);
+        *reinterpret_cast<uint2*>(small + (8 + r) * 128 + off) = make_uint2(lo[0], lo[1]);
+        if (c == 0) ls->qs[r] = qs;
+    }
+    ptx::fence_proxy_async_smem();
+    warp_arrive(&ls->q_full[1]);
+    ptx::named_bar_sync(1 + LANE, 128);                  // the row scales of Q8^T are there
+    float qsc[RC];
+#pragma unroll
+    for (int c = 0; c < RC; ++c) qsc[c] = ls->qs[c] * scale;
+
+    float m_ref[RC], l_part[RC];
+    int limit[RC];
+#pragma unroll
+    for (int c = 0; c < RC; ++c) {
+        m_ref[c] = -INFINITY;
+        l_part[c] = 0.f;
+        limit[c] = c < R ? min(it.kv_end, ctx + it.q_start + (c >> gs) + 1) : 0;
+    }
+    const uint32_t t_row = tmem + (lane_base << 16);
+    // P8^T code (col c, key `row`): B operand [16 rows][128 keys], K-major along keys, one byte per key
+    const uint32_t pchunk = (uint32_t)row >> 4;          // 16-byte chunk of this thread's key byte; swizzled with the row (c & 7)
+    // the row scales of this thread's key, one tile ahead (a dependent pair of global loads: page id, then scales)
+    auto load_scales = [&](int k, float& ks, float& vs) {
+        const int key = it.kv_begin + k * kKeyTile + row;
+        ks = 1.f; vs = 1.f;
+        if (k < n_tiles && key < it.kv_end) {
+            const int64_t pg = bt[key >> 4];
+            const int64_t base = (pg * 2 * sh.Hkv + it.kv_head) * 16 + (key & 15);
+            ks = p.kv_scale[base];
+            vs = p.kv_scale[base + (int64_t)sh.Hkv * 16];
+        }
+    };
+    float ks_n, vs_n;
+    load_scales(0, ks_n, vs_n);
+
+    for (int k = 0; k < n_tiles; ++k) {
+        const int key = it.kv_begin + k * kKeyTile + row;
+        const float ksc = ks_n, vs = vs_n;
+        load_scales(k + 1, ks_n, vs_n);
+        const float lv = __log2f(vs), ivs = 1.f / vs;        // vs is a power of two: both exact
+        const uint32_t buf = gt & 1;
+        ptx::mbar_wait(&ls->s_full[buf], (gt >> 1) & 1);
+        ptx::tc_fence_after();
+        uint32_t sh_[RC], sl_[RC];
+        ptx::tmem_ld<RC>(t_row + col_s(LANE, buf), sh_);
+        ptx::tmem_ld<RC>(t_row + col_s(LANE, buf) + 8, sl_);
+        ptx::tmem_wait_ld();
+        float sv[RC];
+        int* cm = reinterpret_cast<int*>(&ls->cmax[k & 1][swarp][0]);
+#pragma unroll
+        for (int c = 0; c < RC; ++c) {
+            const float raw = fmaf(__uint_as_float(sl_[c]), 0.0625f, __uint_as_float(sh_[c]));
+            sv[c] = key < limit[c] ? fmaf(raw, ksc * qsc[c], lv) : -INFINITY;
+            const int w = __reduce_max_sync(0xffffffffu, ptx::f2ord(sv[c]));
+            if (lane == 0) cm[c] = w;
+        }
+        ptx::named_bar_sync(1 + LANE, 128);
+        bool any_rescale = false;
+        float alpha[RC];
+        const int* cm0 = reinterpret_cast<const int*>(&ls->cmax[k & 1][0][0]);
+#pragma unroll
+        for (int c = 0; c < RC; ++c) {
+            const float m_t = ptx::ord2f(max(max(cm0[c], cm0[16 + c]), max(cm0[32 + c], cm0[48 + c])));
+            alpha[c] = 1.f;
+            if (m_t > m_ref[c] + kRescaleThreshold) {
+                alpha[c] = (m_ref[c] == -INFINITY) ? 0.f : ptx::ex2(m_ref[c] - m_t);
+                m_ref[c] = m_t;
+                any_rescale = true;
+            }
+            const float w = key < limit[c] ? ptx::ex2(sv[c] - m_ref[c]) : 0.f;      // weight p * vs, in (0, 2^8]
+            l_part[c] = l_part[c] * alpha[c] + w * ivs;
+            sv[c] = w;
+        }
+        if (k >= 2) {                                    // PV(gt-2) done: this P8^T buffer is free again
+            ptx::mbar_wait(&ls->pv_done[buf], ((gt - 2) >> 1) & 1);
+        }
+        {
+            uint8_t* ptb = small + 4096 + buf * 4096 + (row & 15);
+#pragma unroll
+            for (int c = 0; c < RC; ++c) {
+                const uint32_t h = e4m3_of(sv[c]);
+                const uint32_t l = e4m3_of((sv[c] - e4m3_value(h)) * 16.f);
+                const uint32_t off = (pchunk ^ (uint32_t)(c & 7)) << 4;
+                ptb[c * 128 + off] = (uint8_t)h;
+                ptb[(8 + c) * 128 + off] = (uint8_t)l;
+            }
+        }
+        if (k > 0 && any_rescale) {                      // uniform over the 128 threads
+            ptx::mbar_wait(&ls->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
+            ptx::tc_fence_after();
+            uint32_t o[RC];
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                ptx::tmem_ld<RC>(t_row + col_o(LANE) + half * 8, o);
+                ptx::tmem_wait_ld();
+#pragma unroll
+                for (int c = 0; c < RC; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha[c]);
+                ptx::tmem_st<RC>(t_row + col_o(LANE) + half * 8, o);
+            }
+            ptx::tmem_wait_st();
+        }
+        ptx::fence_proxy_async_smem();
+        ptx::tc_fence_before();
+        warp_arrive(&ls->p_full[1][gp & 1]);
+        ++gt;
+        ++gp;
+    }
+
+    // ---- column sums over the 128 key lanes
+#pragma unroll
+    for (int c = 0; c < RC; ++c) {
+        float w = l_part[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
+        if (lane == 0) ls->lsum[swarp][c] = w;
+    }
+    ptx::named_bar_sync(1 + LANE, 128);
+    // ---- epilogue: O^T[d = row][c] = hi part + lo part / 16 -> out / workspace
+    ptx::mbar_wait(&ls->pv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
+    ptx::tc_fence_after();
+    uint32_t oh[RC], ol[RC];
+    ptx::tmem_ld<RC>(t_row + col_o(LANE), oh);
+    ptx::tmem_ld<RC>(t_row + col_o(LANE) + 8, ol);
+    ptx::tmem_wait_ld();
+#pragma unroll
+    for (int c = 0; c < RC; ++c) {
+        if (c < R) {
+            const float lc = ls->lsum[0][c] + ls->lsum[1][c] + ls->lsum[2][c] + ls->lsum[3][c];
+            const float o = fmaf(__uint_as_float(ol[c]), 0.0625f, __uint_as_float(oh[c]));
+            if (it.partial_row < 0) {
+                const int tok = tok0 + (c >> gs), head = it.kv_head * G + (c & (G - 1));
+                p.out[((int64_t)tok * sh.Hq + head) * D + row] = __float2bfloat16_rn(__fdividef(o, lc));
+            } else {
+                p.part_o[((int64_t)it.partial_row + c) * D + row] = o;
+                if (row == c) p.part_ml[(int64_t)it.partial_row + c] = make_float2(m_ref[c], lc);
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    ptx::named_bar_sync(1 + LANE, 128);                  // lsum / cmax / qs are reused by the next item
+}
+// ------------------------------------------------------------------------------------------
 template <int LANE, int RC>
 __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p, uint8_t* small, LaneState* ls,
                                              uint32_t tmem, uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base, int swarp) {
@@ -976,7 +1269,7 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
 // ROLE 2: lane S.
 // SPLIT: both warpgroups follow lane 0's item ring; ROLE 0 = warpgroup 0 of the column split (and the swap-kind
 // items), ROLE 2 = warpgroup 1 (swap-kind items are skipped).
-template <int D, int ROLE, bool POLY, bool SPLIT>
+template <int D, int ROLE, bool POLY, bool SPLIT, bool KV8>
 __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Misc* misc, int warp, int lane) {
     using L = Layout<D, SPLIT>;
     constexpr int LANE = (ROLE == 2 && !SPLIT) ? 1 : 0;
@@ -1003,6 +1296,10 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
         if (ROLE == 2 || it.kind == kKindSwap) {
             if constexpr (D == 128) {
                 const int R = it.q_tokens * p.sh.G;
+                if constexpr (KV8) {
+                    if (R <= 4) softmax_swap8<LANE, 4>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
+                    else softmax_swap8<LANE, 8>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
+                } else
                 if (R <= 4) softmax_swap<LANE, 4>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
                 else if (R <= 8) softmax_swap<LANE, 8>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
                 else softmax_swap<LANE, 16>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
@@ -1017,9 +1314,12 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
 // ------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------
-template <int D, bool POLY, bool SPLIT>
+// KV8 (fp8 pools, dual-lane only): tmap = the library's bf16 scratch pool (chunk tiles), tmap8 = the e4m3 pool (decode
+// streams); otherwise tmap = the bf16 pool and tmap8 is a copy of it, unused.
+template <int D, bool POLY, bool SPLIT, bool KV8>
 __global__ void __launch_bounds__(kThreads, 1)
-attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
+attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap8) {
+    static_assert(!(KV8 && (SPLIT || D != 128)), "fp8 pools: dual-lane instantiation, D = 128");
     using L = Layout<D, SPLIT>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -1050,6 +1350,7 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         }
         ptx::fence_barrier_init();
         ptx::prefetch_tmap(&tmap);
+        if (KV8) ptx::prefetch_tmap(&tmap8);
     }
     if (warp == 6) ptx::tmem_alloc(&misc->tmem_base, kTmemCols);
     // Stale shared memory may hold NaN bit patterns, tiles are only partly overwritten by short requests, and
@@ -1070,17 +1371,17 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     // their share to the tile softmax (a 128-column score row in registers) and the decode softmax.
     if (warp < 8) {
         reg_dec<56>();
-        if (warp < kProdT + kProdS) producer<D, SPLIT>(p, &tmap, smem, misc, lane, warp);
-        else if (warp == 5) mma_warp<D, 0, 1, SPLIT>(ptx::smem_u32(smem), misc, lane);     // lane T: score blocks (and swap items); SPLIT: the one issuer
-        else if (SPLIT) { }                                                                 // SPLIT: warps 6, 7 have no role
-        else if (warp == 6) mma_warp<D, 0, 2, false>(ptx::smem_u32(smem), misc, lane);     // lane T: PV blocks
-        else mma_warp<D, 1, 0, false>(ptx::smem_u32(smem), misc, lane);                    // lane S
+        if (warp < kProdT + kProdS) producer<D, SPLIT, KV8>(p, &tmap, &tmap8, smem, misc, lane, warp);
+        else if (warp == 5) mma_warp<D, 0, 1, SPLIT, KV8>(ptx::smem_u32(smem), misc, lane);     // lane T: score blocks (and swap items); SPLIT: the one issuer
+        else if (SPLIT) { }                                                                      // SPLIT: warps 6, 7 have no role
+        else if (warp == 6) mma_warp<D, 0, 2, false, KV8>(ptx::smem_u32(smem), misc, lane);     // lane T: PV blocks
+        else mma_warp<D, 1, 0, false, KV8>(ptx::smem_u32(smem), misc, lane);                    // lane S
     } else if (warp < 12) {
         reg_inc<SPLIT ? 200 : 232>();
-        softmax_warps<D, 0, POLY, SPLIT>(p, smem, misc, warp, lane);
+        softmax_warps<D, 0, POLY, SPLIT, KV8>(p, smem, misc, warp, lane);
     } else {
         reg_inc<SPLIT ? 200 : 160>();
-        softmax_warps<D, 2, SPLIT && POLY, SPLIT>(p, smem, misc, warp, lane);
+        softmax_warps<D, 2, SPLIT && POLY, SPLIT, KV8>(p, smem, misc, warp, lane);
     }
     ptx::tc_fence_before();
     __syncthreads();

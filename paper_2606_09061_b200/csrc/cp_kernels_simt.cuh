@@ -6,6 +6,7 @@
 // Operation defined in include/cp.h / DESIGN.md section 2.
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
 #include "cp_internal.h"
@@ -165,6 +166,137 @@ __global__ void kv_append_rope_kernel(BatchMeta meta, Shape sh, const uint4* __r
             q_rot[row + c] = olo;
             q_rot[row + hc + c] = ohi;
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------
+// N2, second half: FP8 (e4m3) KV pages.  Layout and quantisation rule: include/cp.h
+// (cp_attention_step_fp8) / DESIGN.md R13-R15 / oracle/kv_fp8.py.
+//
+// kv_append_q8_kernel: 16 threads per (token, K|V, kv head) row of D = 128 elements, 8 elements each: row
+// maximum by shuffles, e = the smallest integer with 448 * 2^e >= amax clamped to [-15, 7] -- integer
+// arithmetic on the fp32 fields, the decision oracle/kv_fp8.py takes with frexp -- then x * 2^-e (exact) is
+// rounded to nearest even onto the e4m3 grid, saturating (cvt.rn.satfinite.e4m3x2.f32).  Then the tails of the
+// requests' last pages: codes 0, scales 1.
+// ---------------------------------------------------------------------------------
+__device__ __forceinline__ int64_t slab8_offset(int64_t page, int kv, int head, int Hkv, int B) {
+    return ((page * 2 + kv) * Hkv + head) * (int64_t)B;           // in rows (tokens); x D for codes
+}
+
+__device__ __forceinline__ int e4m3_scale_exponent(float amax) {
+    if (amax == 0.f) return -15;
+    int k;                                                        // amax = f * 2^k, f in [0.5, 1)
+    const float f = frexpf(amax, &k);
+    const int e = (f <= 0.875f) ? k - 9 : k - 8;                  // 448 = 0.875 * 2^9
+    return min(7, max(-15, e));
+}
+
+__device__ __forceinline__ uint32_t e4m3x4(float a, float b, float c, float d) {
+    uint16_t lo, hi;
+    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %2, %1;" : "=h"(lo) : "f"(a), "f"(b));      // upper byte = first operand
+    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %2, %1;" : "=h"(hi) : "f"(c), "f"(d));
+    return (uint32_t)lo | ((uint32_t)hi << 16);
+}
+
+__device__ __forceinline__ void zero_page_tails8(const BatchMeta& meta, const Shape& sh, uint8_t* __restrict__ cache8,
+                                                 float* __restrict__ scales) {
+    const int chunks = sh.D / 16;                                 // 16-byte chunks per row of codes
+    const int64_t total = (int64_t)meta.n_reqs * 2 * sh.Hkv * (sh.B - 1) * chunks;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int c = (int)(i % chunks);
+        int64_t r = i / chunks;
+        const int slot = 1 + (int)(r % (sh.B - 1));
+        r /= (sh.B - 1);
+        const int g = (int)(r % sh.Hkv);
+        r /= sh.Hkv;
+        const int kv = (int)(r & 1);
+        const int req = (int)(r >> 1);
+        const int last = meta.ctx_off[req] + meta.q_len[req] - 1;
+        if (slot <= last % sh.B) continue;
+        const int64_t page = meta.block_table[meta.bt_off[req] + last / sh.B];
+        const int64_t row = slab8_offset(page, kv, g, sh.Hkv, sh.B) + slot;
+        *reinterpret_cast<uint4*>(cache8 + row * sh.D + c * 16) = make_uint4(0, 0, 0, 0);
+        if (c == 0) scales[row] = 1.f;
+    }
+}
+
+__global__ void kv_append_q8_kernel(BatchMeta meta, Shape sh, const uint4* __restrict__ k_new,
+                                    const uint4* __restrict__ v_new, uint8_t* __restrict__ cache8,
+                                    float* __restrict__ scales) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    zero_page_tails8(meta, sh, cache8, scales);
+    // D = 128: 16 threads x 8 elements per row; a warp holds two rows
+    const int64_t total = k_new ? (int64_t)meta.n_tokens * sh.Hkv * 2 * 16 : 0;
+    const int64_t total_pad = (total + 31) & ~(int64_t)31;       // whole warps take part in the shuffles
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total_pad;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const bool live = i < total;
+        const int c = (int)(i & 15);
+        int64_t r = live ? i >> 4 : 0;
+        const int kv = (int)(r & 1);
+        r >>= 1;
+        const int g = (int)(r % sh.Hkv);
+        const int tok = (int)(r / sh.Hkv);
+        const uint4 v = live ? (kv ? v_new : k_new)[((int64_t)tok * sh.Hkv + g) * 16 + c] : make_uint4(0, 0, 0, 0);
+        const __nv_bfloat162* h2 = reinterpret_cast<const __nv_bfloat162*>(&v);
+        float x[8];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { const float2 f = __bfloat1622float2(h2[j]); x[2 * j] = f.x; x[2 * j + 1] = f.y; }
+        float amax = 0.f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) amax = fmaxf(amax, fabsf(x[j]));
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+        const int e = e4m3_scale_exponent(amax);
+        const float inv = __int_as_float((127 - e) << 23);        // 2^-e, exact
+        if (!live) continue;
+        const int req = meta.tok_req[tok];
+        const int pos = meta.ctx_off[req] + (tok - meta.cu_q[req]);
+        const int64_t page = meta.block_table[meta.bt_off[req] + pos / sh.B];
+        const int64_t row = slab8_offset(page, kv, g, sh.Hkv, sh.B) + pos % sh.B;
+        uint2 out;
+        out.x = e4m3x4(x[0] * inv, x[1] * inv, x[2] * inv, x[3] * inv);
+        out.y = e4m3x4(x[4] * inv, x[5] * inv, x[6] * inv, x[7] * inv);
+        *reinterpret_cast<uint2*>(cache8 + row * sh.D + c * 8) = out;
+        if (c == 0) scales[row] = __int_as_float((127 + e) << 23);
+    }
+}
+
+// kv8_dequant_kernel: the pages of every request that has a prefill chunk -> the bf16 scratch pool, page p of
+// request j at scratch page scratch_base[j] + p, same slab layout as a bf16 pool.  code_value * 2^e is exact in
+// bf16 (4 significant bits), so the chunk tiles then compute on exactly the values the fp8 pages hold.  One
+// thread per 16-byte chunk of codes.  Unused slots of a last page were cleared by the append kernel (code 0).
+__global__ void kv8_dequant_kernel(BatchMeta meta, Shape sh, const uint8_t* __restrict__ cache8,
+                                   const float* __restrict__ scales, __nv_bfloat16* __restrict__ scratch,
+                                   int32_t n_scratch_pages) {
+    const int chunks = sh.D / 16;
+    const int64_t per_page = (int64_t)2 * sh.Hkv * sh.B * chunks;
+    const int64_t total = (int64_t)n_scratch_pages * per_page;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int sp = (int)(i / per_page);                       // scratch page
+        const int64_t w = i % per_page;                           // (kv, head, slot, chunk) within the page
+        const int req = meta.scratch_req[sp];
+        const int64_t page = meta.block_table[meta.bt_off[req] + (sp - meta.scratch_base[req])];
+        const int64_t row_in_page = w / chunks;                   // (kv * Hkv + head) * B + slot
+        const int c = (int)(w % chunks);
+        const int64_t src_row = page * 2 * sh.Hkv * sh.B + row_in_page;
+        const uint4 codes = *reinterpret_cast<const uint4*>(cache8 + src_row * sh.D + c * 16);
+        const float sc = scales[src_row];
+        const uint16_t* c2 = reinterpret_cast<const uint16_t*>(&codes);
+        uint4 o[2];
+        __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(o);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            uint32_t h2;
+            asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"(c2[j]));
+            const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h2));
+            ob[j] = __floats2bfloat162_rn(f.x * sc, f.y * sc);
+        }
+        uint4* dst = reinterpret_cast<uint4*>(scratch + ((int64_t)sp * 2 * sh.Hkv * sh.B + row_in_page) * sh.D + c * 16);
+        dst[0] = o[0];
+        dst[1] = o[1];
     }
 }
 

@@ -34,7 +34,7 @@ def test_struct_sizes_match_the_header(lib):
     import ctypes as C
     assert C.sizeof(binding.cp_req_desc) == 32
     assert C.sizeof(binding.cp_latency_row) == 72
-    assert C.sizeof(binding.cp_config) == 72
+    assert C.sizeof(binding.cp_config) == 88
 
 
 def test_missing_library_fails_loudly(tmp_path):
@@ -47,9 +47,9 @@ def test_host_side_argument_errors(lib):
     import ctypes as C
     assert lib.cp_create(None, None) == binding.CP_EINVAL
     assert b"null" in lib.cp_last_error()
-    cfg = binding.cp_config(32, 5, 128, 16, 1, 1024, 0.1, 128, 8, 1024, 0, 0, 1)
+    cfg = binding.cp_config(32, 5, 128, 16, 1, 1024, 0.1, 128, 8, 1024, 0, 0, 0, 0, 0, 0)
     h = C.c_void_p()
     assert lib.cp_create(C.byref(cfg), C.byref(h)) == binding.CP_EINVAL     # Hq % Hkv
-    cfg = binding.cp_config(32, 8, 96, 16, 1, 1024, 0.1, 128, 8, 1024, 0, 0, 1)
+    cfg = binding.cp_config(32, 8, 96, 16, 1, 1024, 0.1, 128, 8, 1024, 0, 0, 0, 0, 0, 0)
     assert lib.cp_create(C.byref(cfg), C.byref(h)) == binding.CP_EINVAL     # head_dim
     assert lib.cp_attention_step(None, 0, None, None, None, None, None, None) == binding.CP_EINVAL
