@@ -191,11 +191,17 @@ def run_ours(args):
     dev = torch.device(f"cuda:{local_rank}")
     build.build()
     spec = wl.CONFIGS[args.workload](seed=rank)           # replicas: same shape, own seed
-    q, k_new, v_new, pool, compact = wl.device_values(spec, dev)
+    fp8 = args.kv_dtype == "e4m3"                          # a separate workload, the headline stays bf16
     n_pages = int(sum(len(b) for b in spec.block_tables))
+    if fp8:
+        q, k_new, v_new, pool, scales, compact, compact_scales = wl.device_values_fp8(spec, dev)
+        chunk_pages = int(sum(len(b) for b, ql in zip(spec.block_tables, spec.q_len) if ql * (spec.Hq // spec.Hkv) > 8))
+    else:
+        q, k_new, v_new, pool, compact = wl.device_values(spec, dev)
     ctx = binding.Context(spec.Hq, spec.Hkv, spec.D, spec.num_blocks, spec.B, sm_scale=spec.sm_scale,
                           max_tokens=spec.T, max_reqs=spec.n_reqs, max_total_pages=n_pages,
-                          device=local_rank)
+                          device=local_rank, kv_dtype=binding.CP_KV_E4M3 if fp8 else binding.CP_KV_BF16,
+                          max_scratch_pages=max(chunk_pages, 1) if fp8 else 0)
     descs, keep = binding.make_descs(spec.q_len, spec.ctx_off, spec.block_tables)
     out = torch.empty((spec.T, spec.Hq, spec.D), device=dev, dtype=torch.bfloat16)
     free_b, total_b = torch.cuda.mem_get_info(dev)
@@ -205,6 +211,9 @@ def run_ours(args):
     if args.rope:                                          # rotary embedding fused into the append
         ctx.cp_enable_rope(binding.rope_inv_freq(spec.D))
     attention_step = ctx.cp_attention_step_rope if args.rope else ctx.cp_attention_step
+    if fp8:
+        attention_step = lambda layer, q_, k_, v_, pool_, out_, stream=None: ctx.cp_attention_step_fp8(
+            layer, q_, k_, v_, pool_, scales, out_, stream=stream)
 
     def step():
         ctx.cp_build_batch(descs=descs, n=spec.n_reqs)
@@ -307,7 +316,7 @@ def run_ours(args):
     tokens_per_s = whole_job_rate(spec.T, args.steps, world, ms_total)
     # roofline for the step's kernels (append + attention + combine), CUDA events on the launch stream
     attn_us = float(np.mean(step_us)) if len(step_us) else ms_per_step * 1e3
-    bytes_alg, flops_alg = spec.algorithmic_bytes(), spec.flops()
+    bytes_alg, flops_alg = spec.algorithmic_bytes(args.kv_dtype), spec.flops()
     t_hbm = bytes_alg / (peaks["hbm_gbs"] * 1e9)
     # the tensor peak that applies (B200_PROFILING.md): the burst figure for a kernel timed alone for a short while,
     # the sustained one when the timed region is long enough for the power cap to engage (>= 1 s, or sw_power_cap seen)
@@ -319,12 +328,12 @@ def run_ours(args):
         achieved, peak, runit = bytes_alg / (attn_us * 1e-6) / 1e9, peaks["hbm_gbs"], "GB/s"
     else:
         achieved, peak, runit = flops_alg / (attn_us * 1e-6) / 1e12, tc_peak, "TFLOP/s"
-    traffic, traffic_source = ncu_traffic(spec.name)
+    traffic, traffic_source = ncu_traffic(spec.name + ("_e4m3" if fp8 else ""))
     res = {
         "metric": METRIC, "value": tokens_per_s, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": config_dict(spec),
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16" if not fp8 else "bf16 (fp8 e4m3 KV pages)", "data": "synthetic",
+        "config": config_dict(spec, args.kv_dtype),
         "launch": {"parallelism": "replicas" if world > 1 else "single", "rope": bool(args.rope),
                    "work_items": info.n_work_items, "combine_items": info.n_combine_items,
                    "grid_attn": info.grid_attn, "kernels_per_step": info.kernels_per_step},
@@ -352,7 +361,7 @@ def run_ours(args):
                      "t_hbm_us": t_hbm * 1e6, "t_tensor_us": t_tc * 1e6,
                      "frac_nominal_8TBs_2250TF": max(bytes_alg / 8e12, flops_alg / 2.25e15) / (attn_us * 1e-6)},
     }
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and not fp8:
         from oracle import attention as ora
         cache = compact.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
         kb = k_new.view(torch.int16).cpu().numpy().view(np.uint16)
@@ -418,6 +427,8 @@ def main():
     ap.add_argument("--workload", default="b2048", choices=sorted(wl.CONFIGS))
     ap.add_argument("--rope", action="store_true",
                     help="time cp_attention_step_rope (rotary embedding of Q / new K fused into the append)")
+    ap.add_argument("--kv-dtype", default="bf16", choices=["bf16", "e4m3"],
+                    help="e4m3: FP8 KV pages through cp_attention_step_fp8 (its own algorithmic-bytes roofline)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

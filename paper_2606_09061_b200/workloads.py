@@ -86,8 +86,10 @@ class BatchSpec:
     def flops(self) -> int:
         return 4 * self.D * self.Hq * self.causal_pairs()
 
-    def algorithmic_bytes(self) -> int:
-        kv = int(2 * self.kv_len.sum() * self.Hkv * self.D * 2)
+    def algorithmic_bytes(self, kv_dtype: str = "bf16") -> int:
+        # fp8 pages: one byte per element + one fp32 scale per (token, KV head, K|V) row
+        row = self.D * 2 if kv_dtype == "bf16" else self.D + 4
+        kv = int(2 * self.kv_len.sum() * self.Hkv * row)
         qo = 2 * self.T * self.Hq * self.D * 2
         tables = 4 * int(sum(len(b) for b in self.block_tables))
         return kv + qo + tables
@@ -308,6 +310,44 @@ def device_values(spec: BatchSpec, device, seed: Optional[int] = None,
             pool.view(torch.int16).fill_(pv)
     pool[touched] = compact
     return q, k_new, v_new, pool, compact
+
+
+def device_values_fp8(spec: BatchSpec, device, seed: Optional[int] = None):
+    """FP8 (e4m3) pool for the large configs, generated ON THE GPU with a seeded torch generator: q / k_new / v_new
+    bf16 N(0,1) as in device_values; the touched pages hold uniformly random finite e4m3 codes with the row scale
+    2^-7 (|value| <= 3.5); slots at positions >= ctx_off and every untouched page hold NaN codes (0x7F) / whatever
+    torch.empty left.  Returns (q, k_new, v_new, codes_pool u8 [num_blocks,2,Hkv,B,D], scales_pool f32
+    [num_blocks,2,Hkv,B], compact_codes, compact_scales) -- the compact copies are the state BEFORE the step."""
+    import torch
+    g = torch.Generator(device=device)
+    g.manual_seed((spec.seed if seed is None else seed) + 0xF8)
+    T, Hq, Hkv, D, B = spec.T, spec.Hq, spec.Hkv, spec.D, spec.B
+    q = torch.randn((T, Hq, D), generator=g, device=device, dtype=torch.float32).bfloat16()
+    k_new = torch.randn((T, Hkv, D), generator=g, device=device, dtype=torch.float32).bfloat16()
+    v_new = torch.randn((T, Hkv, D), generator=g, device=device, dtype=torch.float32).bfloat16()
+    touched = torch.from_numpy(spec.touched_pages().astype(np.int64)).to(device)
+    n_touched = int(touched.numel())
+    mag = torch.randint(0, 0x7F, (n_touched, 2, Hkv, B, D), generator=g, device=device, dtype=torch.int16)
+    sign = torch.randint(0, 2, (n_touched, 2, Hkv, B, D), generator=g, device=device, dtype=torch.int16)
+    compact_codes = (mag | (sign << 7)).to(torch.uint8)
+    del mag, sign
+    compact_scales = torch.full((n_touched, 2, Hkv, B), 2.0 ** -7, device=device, dtype=torch.float32)
+    base = 0
+    for bt, off in zip(spec.block_tables, spec.ctx_off):
+        off = int(off)
+        first = off // B
+        if first < len(bt):
+            compact_codes[base + first, :, :, off - first * B:, :] = 0x7F
+            compact_scales[base + first, :, :, off - first * B:] = float("nan")
+            if first + 1 < len(bt):
+                compact_codes[base + first + 1:base + len(bt)] = 0x7F
+                compact_scales[base + first + 1:base + len(bt)] = float("nan")
+        base += len(bt)
+    codes = torch.empty((spec.num_blocks, 2, Hkv, B, D), device=device, dtype=torch.uint8)
+    scales = torch.empty((spec.num_blocks, 2, Hkv, B), device=device, dtype=torch.float32)
+    codes[touched] = compact_codes
+    scales[touched] = compact_scales
+    return q, k_new, v_new, codes, scales, compact_codes, compact_scales
 
 
 # ----------------------------------------------------------------------------
