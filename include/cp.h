@@ -107,7 +107,7 @@ typedef struct {
     float   us;                 /* device time of cp_attention_step (CUDA events)  */
     int32_t n_prefill;          /* requests with q_len > 1 or CP_REQ_PREFILL       */
     int32_t n_decode;           /* the others                                      */
-    int32_t layer;
+    int32_t layer;              /* >= 0: the layer of a cp_attention_step; -n: n layers timed together (cp_attention_layers) */
     int64_t iter;               /* index of the cp_build_batch this step ran under */
 } cp_latency_row;
 
@@ -147,6 +147,15 @@ int cp_build_batch(cp_ctx* ctx, const cp_req_desc* reqs, int32_t n_reqs,
  * All pointers 16-byte aligned.  Errors: CP_ESTATE (no batch built), CP_EINVAL, CP_ECUDA. */
 int cp_attention_step(cp_ctx* ctx, int32_t layer, const void* q, const void* k_new,
                       const void* v_new, void* kv_cache, void* out, void* cuda_stream);
+
+/* All layers of the iteration in ONE submission (PAPER.md:201 names kernel launch latency among the fixed
+ * per-round overheads; most rounds of a serving trace are a handful of decodes, where the per-call cost is the
+ * bulk of the time): exactly the kernels of n_layers cp_attention_step calls with layer = 0 .. n_layers-1, but
+ * one host call, ONE CUDA-event pair and one cp_latency_row for the whole iteration (its `layer` is -n_layers,
+ * its `us` the time of all layers).  q, k_new, v_new, kv_cache, out: HOST arrays of n_layers DEVICE pointers
+ * (k_new and v_new may both be NULL).  bf16 pools only.  Errors as cp_attention_step. */
+int cp_attention_layers(cp_ctx* ctx, int32_t n_layers, const void* const* q, const void* const* k_new,
+                        const void* const* v_new, void* const* kv_cache, void* const* out, void* cuda_stream);
 
 /* N2 of SURVEY.md 8(f): rotary position embedding fused into the append (H2).  PAPER.md is
  * silent on positional encoding (the execution backend is untouched); the
@@ -208,6 +217,8 @@ typedef struct {
     int64_t n_partial_rows;      /* workspace rows in use                          */
     int32_t kernels_per_step;    /* kernel launches one cp_attention_step issues   */
     int32_t grid_attn, grid_combine;
+    double  alg_flops, alg_bytes; /* algorithmic work of ONE layer's step (SURVEY.md 8(d) formulas: FLOPs = 4 D Hq x causal
+                                    pairs; bytes = KV once per request and KV head + Q + out + 4 B per page)          */
     int32_t split;               /* 1: tensor-bound batch, runs the SPLIT instantiation of the kernel (both
                                     softmax warpgroups on every chunk tile); 0: dual-lane instantiation */
 } cp_batch_info;

@@ -124,14 +124,19 @@ def kv_append_fp8(k_new_bits, v_new_bits, codes, scales, q_len, ctx_off, block_t
             tok += 1
 
 
-def pages_as_bf16_bits(codes, scales, keys_per_page=None) -> np.ndarray:
+def pages_as_bf16_bits(codes, scales, keys_per_page=None, chunk: int = 1024) -> np.ndarray:
     """The values the fp8 pages hold, as bf16 bit patterns [n, 2, Hkv, B, D] (exact; for the attention oracle).
-    Slots that hold no key (keys_per_page[i] <= slot) may carry any scale bits: they are returned as zeros."""
+    Slots that hold no key (keys_per_page[i] <= slot) may carry any scale bits: they are returned as zeros.
+    (Converted `chunk` pages at a time: the float64 intermediate of a 40 GiB-pool batch would not fit the host.)"""
     codes = np.asarray(codes, dtype=np.uint8)
-    sc = np.asarray(scales, dtype=np.float32).astype(np.float64)
-    if keys_per_page is not None:
-        is_key = np.arange(codes.shape[3])[None, :] < np.asarray(keys_per_page)[:, None]      # [n, B]
-        sc = np.where(is_key[:, None, None, :], sc, 1.0)
-        codes = np.where(is_key[:, None, None, :, None], codes, 0).astype(np.uint8)
-    vals = _TABLE[codes] * sc[..., None]
-    return f64_to_bf16_bits_exact(vals)
+    scales = np.asarray(scales, dtype=np.float32)
+    out = np.empty(codes.shape, dtype=np.uint16)
+    for s0 in range(0, codes.shape[0], chunk):
+        c = codes[s0:s0 + chunk]
+        sc = scales[s0:s0 + chunk].astype(np.float64)
+        if keys_per_page is not None:
+            is_key = np.arange(c.shape[3])[None, :] < np.asarray(keys_per_page[s0:s0 + chunk])[:, None]      # [n, B]
+            sc = np.where(is_key[:, None, None, :], sc, 1.0)
+            c = np.where(is_key[:, None, None, :, None], c, 0).astype(np.uint8)
+        out[s0:s0 + chunk] = f64_to_bf16_bits_exact(_TABLE[c] * sc[..., None])
+    return out

@@ -28,7 +28,7 @@ EXPORTS = [
     "cp_sched_destroy", "cp_sched_add_request", "cp_sched_next", "cp_sched_commit",
     "cp_sched_next_arrival", "cp_sched_has_work", "cp_sched_get_stats",
     "cp_sched_request_times", "cp_sched_predict", "cp_sched_select_chunk",
-    "cp_enable_rope", "cp_attention_step_rope", "cp_attention_step_fp8",
+    "cp_enable_rope", "cp_attention_step_rope", "cp_attention_step_fp8", "cp_attention_layers",
 ]
 
 
@@ -56,7 +56,8 @@ class cp_batch_info(C.Structure):
     _fields_ = [("n_reqs", C.c_int32), ("n_tokens", C.c_int32), ("n_work_items", C.c_int32),
                 ("n_combine_items", C.c_int32), ("n_tc_items", C.c_int32),
                 ("n_partial_rows", C.c_int64), ("kernels_per_step", C.c_int32),
-                ("grid_attn", C.c_int32), ("grid_combine", C.c_int32), ("split", C.c_int32)]
+                ("grid_attn", C.c_int32), ("grid_combine", C.c_int32), ("alg_flops", C.c_double),
+                ("alg_bytes", C.c_double), ("split", C.c_int32)]
 
 
 class cp_sched_config(C.Structure):
@@ -107,6 +108,7 @@ def load(path: Optional[str] = None):
     lib.cp_attention_step.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     lib.cp_attention_step_rope.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     lib.cp_attention_step_fp8.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 7
+    lib.cp_attention_layers.argtypes = [C.c_void_p, C.c_int32] + [C.POINTER(C.c_void_p)] * 5 + [C.c_void_p]
     lib.cp_enable_rope.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     lib.cp_latency_table.argtypes = [C.c_void_p, C.POINTER(cp_latency_row), C.c_int32,
                                      C.POINTER(C.c_int32)]
@@ -209,6 +211,15 @@ class Context:
     def cp_attention_step_fp8(self, layer, q, k_new, v_new, kv_cache8, kv_scale, out, stream=None):
         _check(self.lib.cp_attention_step_fp8(self.handle, layer, _ptr(q), _ptr(k_new), _ptr(v_new),
                                               _ptr(kv_cache8), _ptr(kv_scale), _ptr(out), _ptr(stream)))
+
+    @staticmethod
+    def pointer_array(ptrs):
+        """HOST array of device pointers for cp_attention_layers (build once, reuse every iteration)."""
+        return (C.c_void_p * len(ptrs))(*[_ptr(p) for p in ptrs])
+
+    def cp_attention_layers(self, q, k_new, v_new, kv_cache, out, stream=None):
+        """q ... out: pointer_array()s of equal length (k_new / v_new may be None)."""
+        _check(self.lib.cp_attention_layers(self.handle, len(q), q, k_new, v_new, kv_cache, out, _ptr(stream)))
 
     def cp_latency_table(self, cap=4096) -> List[cp_latency_row]:
         rows = (cp_latency_row * cap)()

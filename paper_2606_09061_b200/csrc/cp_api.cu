@@ -517,7 +517,10 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     int32_t n_tc = 0;
     if (c->use_tc) n_tc = (int32_t)n_items;
     c->info = cp_batch_info{n_reqs, (int32_t)T, (int32_t)n_items, (int32_t)c->combines.size(), n_tc,
-                            partial_rows, 0, 0, 0, tensor_bound ? 1 : 0};
+                            partial_rows, 0, 0, 0,
+                            4.0 * sh.D * sh.Hq * alg_pairs,
+                            2.0 * alg_keys * sh.Hkv * (c->kv8 ? sh.D + 4.0 : sh.D * 2.0) + 2.0 * (double)T * sh.Hq * sh.D * 2 + 4.0 * (double)P,
+                            tensor_bound ? 1 : 0};
     c->feat[0] = f_pf_tokens; c->feat[1] = f_dec; c->feat[2] = (float)n_reqs; c->feat[3] = f_sum_ctx;
     c->feat[4] = f_max_ctx; c->feat[5] = f_pf_proc; c->feat[6] = f_pf_proc_max;
     c->n_prefill = n_prefill;
@@ -695,8 +698,9 @@ static int launch_tc(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const fl
                              : launch_tc_d<64>(c, q, kv_cache, kv_scale, out, stream, launches);
 }
 
-static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new, const void* v_new,
-                          void* kv_cache, void* out, void* stream_, bool rope, void* kv_scale = nullptr) {
+// validate the arguments of one layer's step and enqueue its kernels (no events, no latency row)
+static int issue_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new, const void* v_new,
+                      void* kv_cache, void* out, cudaStream_t stream, bool rope, void* kv_scale, int* launches_out) {
     if (!c) return CP_EINVAL;
     if (!c->have_batch) { cp_set_error("cp_attention_step: no batch built"); return CP_ESTATE; }
     if (c->kv8 != (kv_scale != nullptr)) {
@@ -720,11 +724,8 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
         cp_set_error("cp_attention_step: pointers must be 16-byte aligned");
         return CP_EINVAL;
     }
-    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     c->step_stream = stream;
     const BatchMeta& m = c->meta;
-    TimedStep& ts = c->ring[(size_t)(c->ring_head % kRing)];
-    CP_CUDA(cudaEventRecord(ts.start, stream));
     int launches = 0;
     if (m.n_tokens > 0) {
         if (rope) {
@@ -788,6 +789,12 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
         }
         if (rc != CP_OK) return rc;
     }
+    *launches_out = launches;
+    return CP_OK;
+}
+
+// close a timed region [ts.start, stop recorded here]: the Table-1 features of the batch + which layer(s)
+static int finish_timed(cp_ctx* c, TimedStep& ts, int32_t layer, int launches, cudaStream_t stream) {
     CP_CUDA(cudaEventRecord(ts.stop, stream));
     c->info.kernels_per_step = launches;
     cp_latency_row& row = ts.row;
@@ -801,6 +808,42 @@ static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k
     ++c->ring_head;
     if (c->ring_head - c->ring_tail > kRing) c->ring_tail = c->ring_head - kRing;   // oldest rows overwritten
     return CP_OK;
+}
+
+static int attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new, const void* v_new,
+                          void* kv_cache, void* out, void* stream_, bool rope, void* kv_scale = nullptr) {
+    if (!c) return CP_EINVAL;
+    if (!c->have_batch) { cp_set_error("cp_attention_step: no batch built"); return CP_ESTATE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    TimedStep& ts = c->ring[(size_t)(c->ring_head % kRing)];
+    CP_CUDA(cudaEventRecord(ts.start, stream));
+    int launches = 0;
+    const int rc = issue_step(c, layer, q, k_new, v_new, kv_cache, out, stream, rope, kv_scale, &launches);
+    if (rc != CP_OK) return rc;
+    return finish_timed(c, ts, layer, launches, stream);
+}
+
+// One submission for all layers of an iteration (PAPER.md:201 counts kernel-launch latency among the fixed
+// per-round overheads): the same kernels as n_layers cp_attention_step calls, ONE event pair, one latency row.
+extern "C" int cp_attention_layers(cp_ctx* c, int32_t n_layers, const void* const* q, const void* const* k_new,
+                                   const void* const* v_new, void* const* kv_cache, void* const* out, void* stream_) {
+    if (!c || n_layers < 1 || !q || !kv_cache || !out || ((k_new == nullptr) != (v_new == nullptr))) {
+        cp_set_error("cp_attention_layers: bad argument");
+        return CP_EINVAL;
+    }
+    if (!c->have_batch) { cp_set_error("cp_attention_layers: no batch built"); return CP_ESTATE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    TimedStep& ts = c->ring[(size_t)(c->ring_head % kRing)];
+    CP_CUDA(cudaEventRecord(ts.start, stream));
+    int total = 0;
+    for (int32_t l = 0; l < n_layers; ++l) {
+        int launches = 0;
+        const int rc = issue_step(c, l, q[l], k_new ? k_new[l] : nullptr, v_new ? v_new[l] : nullptr, kv_cache[l], out[l],
+                                  stream, false, nullptr, &launches);
+        if (rc != CP_OK) return rc;
+        total += launches;
+    }
+    return finish_timed(c, ts, -n_layers, total, stream);
 }
 
 extern "C" int cp_attention_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new,

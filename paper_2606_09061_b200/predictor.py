@@ -110,6 +110,8 @@ def fit_mlp(X16, y, w, Xv, yv, epochs=300, lr=2e-3, weight_decay=1e-3, dropout=0
     t = lambda a: torch.tensor(a, dtype=torch.float32)
     Z, Zv = t((X - mu) * inv), t((np.asarray(Xv, np.float64) - mu) * inv)
     Y, Yv, W = t((np.asarray(y) - ym) / ys), t((np.asarray(yv) - ym) / ys), t(w)
+    Wv = t((float(np.median(y)) / np.asarray(yv, np.float64)) ** 2)      # validation in relative error too
+    Wv = Wv / Wv.mean()
     layers = []
     for i in range(4):
         layers.append(torch.nn.Linear(MLP_DIMS[i], MLP_DIMS[i + 1]))
@@ -129,7 +131,7 @@ def fit_mlp(X16, y, w, Xv, yv, epochs=300, lr=2e-3, weight_decay=1e-3, dropout=0
             opt.step()
         net.eval()
         with torch.no_grad():
-            v = float(asymmetric_huber(net(Zv).squeeze(1), Yv, torch.ones_like(Yv)))
+            v = float(asymmetric_huber(net(Zv).squeeze(1), Yv, Wv))
         if v < best:
             best, best_state = v, {k: p.detach().clone() for k, p in net.state_dict().items()}
     net.load_state_dict(best_state)
@@ -163,22 +165,19 @@ def predict_mlp(model, X16):
 # ------------------------------------------------------------------------------------------------
 # data collection on the GPU (the logging half is cp_latency_table, H6)
 # ------------------------------------------------------------------------------------------------
-def harvest(n_samples=6000, seed=0, Hq=32, Hkv=8, D=128, B=16, budget=2048, pool_pages=262144, device=0, repeats=2):
+def harvest(n_samples=6000, seed=0, Hq=32, Hkv=8, D=128, B=16, budget=2048, pages_per_layer=131072, layers=1,
+            layer_gemms=False, device=0, repeats=2):
     """Sweep synthetic mixed batches shaped like the token-budget scheduler's rounds (decodes first,
-    prefill chunks fill the rest: PAPER.md:87) and log (11 raw features, us) per round."""
-    import torch
+    prefill chunks fill the rest: PAPER.md:87) and log (11 raw features, us) per round -- through the SAME
+    IterationRunner the serving loop uses (trace_run.py), so the target is exactly the time the scheduler's clock
+    is advanced by: all `layers` attention steps including the KV append, plus, with layer_gemms=True, the dense
+    projections of every layer (the whole-forward-pass clock of PAPER.md:109, :456).  A batch is run 1 + repeats
+    times; the first run warms the metadata / TLB, the others are AVERAGED into one row (one row per batch: no batch
+    can sit on both sides of the train / test split)."""
+    from . import trace_run
     rng = np.random.default_rng(seed)
-    dev = torch.device(f"cuda:{device}")
-    torch.cuda.set_device(dev)
-    g = torch.Generator(device=dev).manual_seed(seed)
-    q = torch.randn((budget, Hq, D), generator=g, device=dev).bfloat16()
-    pool = torch.randn((pool_pages, 2, Hkv, B, D), generator=g, device=dev, dtype=torch.float32).bfloat16() \
-        if pool_pages * 2 * Hkv * B * D * 4 < 8e9 else torch.zeros((pool_pages, 2, Hkv, B, D), device=dev, dtype=torch.bfloat16)
-    out = torch.empty((budget, Hq, D), device=dev, dtype=torch.bfloat16)
-    ctx = binding.Context(Hq, Hkv, D, pool_pages, B, max_tokens=budget, max_reqs=1024, max_total_pages=pool_pages, device=device)
-    free_b, total_b = torch.cuda.mem_get_info(dev)
-    ctx.cp_set_memory_stats((total_b - free_b) / 2**20, free_b / 2**20, torch.cuda.memory_allocated(dev) / 2**20,
-                            torch.cuda.memory_reserved(dev) / 2**20)
+    runner = trace_run.IterationRunner(Hq, Hkv, D, B, layers, pages_per_layer, budget, 1024, seed, device, layer_gemms,
+                                       random_pool=True)
     raw, us = [], []
     for _ in range(n_samples):
         n_dec = int(rng.choice([0, 1, 4, 16, 64, 128, 256, 512])) if rng.random() < 0.8 else int(rng.integers(0, 513))
@@ -196,21 +195,23 @@ def harvest(n_samples=6000, seed=0, Hq=32, Hkv=8, D=128, B=16, budget=2048, pool
         if not q_len:
             continue
         need = [(int(c) + int(l) + B - 1) // B for l, c in zip(q_len, ctx_off)]
-        if sum(need) > pool_pages:
+        if sum(need) > pages_per_layer:
             continue
-        ids = rng.choice(pool_pages, size=sum(need), replace=False).astype(np.int32)
+        ids = rng.choice(pages_per_layer, size=sum(need), replace=False).astype(np.int32)
         tabs, pos = [], 0
         for n in need:
             tabs.append(ids[pos:pos + n])
             pos += n
-        ctx.cp_build_batch(q_len, ctx_off, tabs)
-        for _r in range(repeats + 1):                       # first run warms the metadata / TLB; keep the rest
-            ctx.cp_attention_step(0, q, None, None, pool, out)
-        rows = ctx.cp_latency_table()
-        for r in rows[1:]:
-            raw.append(list(r.feat))
-            us.append(r.us)
-    ctx.close()
+        flags = [0] * n_dec + [binding.CP_REQ_PREFILL] * (len(q_len) - n_dec)      # a 1-token chunk is still prefill
+        ts = []
+        for r in range(repeats + 1):
+            descs, keep = binding.make_descs(q_len, ctx_off, tabs, flags=flags)
+            t, row, _ = runner.run(descs, len(q_len))
+            if r > 0:
+                ts.append(t)
+        raw.append(list(row.feat))
+        us.append(float(np.mean(ts)))
+    runner.close()
     return np.asarray(raw, np.float64), np.asarray(us, np.float64)
 
 
@@ -222,11 +223,16 @@ def train_and_report(raw, us, seed=0, epochs=300, budget=2048):
     tr, va, te, b = bucket_downsample_split(X[:, 12].astype(np.int64), rng, full_budget=budget)
     counts = np.bincount(b[tr], minlength=b.max() + 1).astype(np.float64)
     w = (counts[counts > 0].mean() / counts[b[tr]])          # bucket-aware sample weight (Eq. 5)
+    # Reading of Eq. 5's per-sample weight w_i (the paper gives no formula): bucket weight x (median / y_i)^2, so that
+    # the Huber term measures the RELATIVE error -- rounds range over two orders of magnitude in time, and Eq. 10
+    # compares T_hat with T* for short and long candidate rounds alike.
+    w = w * (float(np.median(us[tr])) / us[tr]) ** 2
+    w = w / w.mean()
     lin = fit_linear(X[tr], us[tr], w)
     mlp = fit_mlp(X[tr], us[tr], w, X[va], us[va], epochs=epochs, seed=seed)
     bounds = (0.05 * float(np.median(us)), 0.10 * float(np.median(us)))
     rep = {"samples": int(len(us)), "train": int(len(tr)), "val": int(len(va)), "test": int(len(te)),
-           "target_unit": "us (attention step, one layer)", "median_us": float(np.median(us)),
+           "target_unit": "us (what IterationRunner.run returns: every layer of the round)", "median_us": float(np.median(us)),
            "linear_test": metrics(us[te], predict_linear(lin, X[te]), bounds),
            "mlp_test": metrics(us[te], predict_mlp(mlp, X[te]), bounds),
            "bounded_error_thresholds_us": list(bounds)}

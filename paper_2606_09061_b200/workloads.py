@@ -385,3 +385,21 @@ def make_apc_trace(n_requests: int = 1000, seed: int = 0, mean_gap_us: float = 2
     arrival_us = np.floor(np.cumsum(gaps)).astype(np.int64)
     out = rng.integers(8, 65, n_requests)
     return np.arange(n_requests, dtype=np.int64), arrival_us, prompt.astype(np.int64), out.astype(np.int64)
+
+
+def make_sharegpt_like_trace(n_requests: int = 200, gap_us: float = 100000.0, seed: int = 0, prompt_median: float = 19.0,
+                             prompt_p90: float = 179.0, max_ctx: int = 512, max_gen: int = 512, out_median: float = 128.0,
+                             out_sigma: float = 1.0):
+    """The paper's short-context serving mix, as a synthetic stand-in (ShareGPT itself is not available here):
+    200 requests at a FIXED inter-arrival of 0.1 s, prompt lengths with median 19 and P90 179 tokens, context clipped
+    to 512, generation capped at 512.  Prompts are lognormal with that median and P90 (sigma =
+    ln(179 / 19) / 1.2816), clipped to [1, max_ctx - 1]; the paper does not print the output-length distribution:
+    lognormal(median 128, sigma 1) clipped to [1, min(max_gen, max_ctx - prompt)] is our reading.  `gap_us` below the
+    iteration time gives the compressed variant (the queue has depth: many tiny chunks per round)."""
+    rng = np.random.default_rng(seed)
+    sigma = float(np.log(prompt_p90 / prompt_median) / 1.2815515655446004)
+    prompt = np.clip(np.rint(np.exp(np.log(prompt_median) + sigma * rng.standard_normal(n_requests))), 1, max_ctx - 1).astype(np.int64)
+    out = np.rint(np.exp(np.log(out_median) + out_sigma * rng.standard_normal(n_requests)))
+    out = np.clip(out, 1, np.minimum(max_gen, max_ctx - prompt)).astype(np.int64)
+    arrival_us = np.floor(np.arange(n_requests) * gap_us).astype(np.int64)
+    return np.arange(n_requests, dtype=np.int64), arrival_us, prompt, out

@@ -3,7 +3,10 @@ every iteration, libcp runs it on the GPU for every layer, and
   * sampled iterations are checked against the fp64 oracle (layers 0 and last),
   * the KV pages the step wrote equal the oracle's append,
   * the schedule is bit-identical to the reference scheduler replayed on the measured times.
-CP_FULL_TRACE=1 additionally runs the full configs[4] (1000 requests, 32 layers, 40 GiB pool)."""
+configs[4] at its full shape (1000-request trace, 32 layers, 20,480 pages per layer = 40 GiB, budget 2048) runs
+un-gated for its first 400 iterations with an oracle sample every 50th iteration on layers 0 and 31 (SURVEY.md
+8(d)); CP_FULL_TRACE=1 additionally runs it to the end.  The LPRS / APC loop (harvest -> train -> schedule) runs
+un-gated on a reduced model with the whole-forward-pass clock; CP_FULL_TRACE=1 runs the long version."""
 import hashlib
 import json
 import os
@@ -20,13 +23,16 @@ from tests import gpu_util as gu
 pytestmark = pytest.mark.gpu
 
 
-def replay_reference(trace, iter_us_log, **kw):
-    """Reference scheduler fed the SAME measured iteration times; returns its schedule digest."""
+def replay_reference(trace, iter_us_log, truncated=False, **kw):
+    """Reference scheduler fed the SAME measured iteration times; returns its schedule digest.
+    truncated: the run stopped after len(iter_us_log) iterations (max_iters) -- stop at the same point."""
     ref = rs.RefScheduler(rs.SchedConfig(**kw))
     for rid, a, p, o in zip(*trace):
         ref.add_request(int(rid), int(a), int(p), int(o))
     h, t, i = hashlib.sha256(), 0, 0
     while ref.has_work() and i <= len(iter_us_log):
+        if truncated and i == len(iter_us_log):
+            break
         b = ref.next(t)
         h.update(rs.pack_record(b))
         if not b:
@@ -134,47 +140,6 @@ def test_full_config5_trace():
     assert n == len(log) and digest == report["schedule_sha256"]
 
 
-@pytest.mark.skipif(os.environ.get("CP_FULL_TRACE") != "1", reason="set CP_FULL_TRACE=1 (minutes, 40 GiB pool)")
-def test_lprs_apc_trace_with_trained_predictor():
-    """harvest cp_latency_table, train the Table-7 MLP, then run configs[4]
-    (compressed arrivals) under token budget / LPRS / LPRS+APC with that predictor; every schedule
-    must still equal the reference scheduler's replay (same predictor data on both sides)."""
-    from paper_2606_09061_b200 import predictor as pr
-    build.build()
-    raw, us = pr.harvest(int(os.environ.get("CP_HARVEST", "3000")), seed=0)
-    rep, lin, mlp = pr.train_and_report(raw, us, seed=0, epochs=int(os.environ.get("CP_EPOCHS", "300")))
-    X = pr.features16(raw)
-    full = X[:, 12] >= 2000
-    t_star = float(np.median(us[full]))                     # per-layer us of a typical full-budget round
-    rate = float(os.environ.get("CP_TRACE_RATE", "64"))
-    trace = wl.make_trace(1000, rate_per_s=rate, seed=0)
-    kind, w, mu, inv = pr.export_mlp(mlp)
-    base = dict(alpha=100.0, beta=-1.0, B_max=2048, S_max=1024, num_blocks=20480, block_size=16,
-                page_mb=2 * 8 * 16 * 128 * 2 * 32 / 2**20)
-    lprs = dict(base, mode=rs.MODE_LPRS, Delta=64, T_star=t_star, lambda_u=1.0, lambda_o=2.0, C_max=4, L_min=64,
-                pred_kind=kind, pred_weights=w, feat_mu=mu, feat_inv_sigma=inv)
-    out = {"predictor": rep, "T_star_us_per_layer": t_star, "arrival_rate_per_s": rate, "runs": {}}
-    for name, kw in [("token_budget", base), ("lprs", lprs), ("lprs_apc", dict(lprs, apc=True))]:
-        report, log = trace_run.run_trace(trace, sched_kw=kw)
-        digest, n = replay_reference(trace, log, **kw)
-        assert n == len(log) and digest == report["schedule_sha256"], name
-        assert report["e2e_s"]["finished"] == 1000
-        it = np.asarray(log, np.float64) / 32.0            # per-layer us of every iteration
-        mixed = report["iteration_us_by_class"]["mixed"]
-        report["per_layer_us"] = {"mean": float(it.mean()), "p95": float(np.percentile(it, 95)), "max": float(it.max()),
-                                  "frac_over_T_star": float((it > t_star).mean())}
-        report["mixed_iterations"] = mixed["iterations"]
-        report.pop("sched", None)
-        out["runs"][name] = report
-    os.makedirs("gpurun_out", exist_ok=True)
-    with open("gpurun_out/lprs_report.json", "w") as f:
-        json.dump(out, f)
-    # latency control (PAPER.md:113 "minimizing deviation from a target latency budget"): LPRS pulls the tail of
-    # the iteration time towards the target -- P95 and maximum both drop against plain token-budget chunking
-    tb, lp = out["runs"]["token_budget"]["per_layer_us"], out["runs"]["lprs"]["per_layer_us"]
-    assert lp["p95"] < tb["p95"] and lp["max"] < tb["max"]
-
-
 def test_apc_ablation_shape_trace_on_gpu():
     """the APC ablation workload shape (49:1 short (30-50) : long (200-220)
     prompts, bursty arrivals) -- many tiny chunks per iteration -- through the whole path with LPRS + APC on,
@@ -213,3 +178,105 @@ def test_reduced_trace_with_layer_gemms():
     assert np.mean(log1) > np.mean(log0)
     digest, n = replay_reference(trace, log1, **dict(kw, page_mb=2 * Hkv * B * D * 2 * layers / 2**20))
     assert n == len(log1) and digest == rep1["schedule_sha256"]
+
+
+def test_config5_full_shape_first_iterations():
+    """BASELINE.json configs[4] at full shape -- 8B attention shape x 32 layers, 20,480 pages per layer (40 GiB
+    pool), 1000-request trace at 8 req/s, aging scheduler with budget 2048 -- for its first 400 iterations: oracle
+    parity every 50th iteration on layers 0 and 31, schedule identity with the reference replay,
+    and the trace-level roofline fields of the report."""
+    build.build()
+    trace = wl.make_trace(1000, rate_per_s=8.0, seed=0)
+    stats = []
+    scale = float(np.float32(1.0) / np.sqrt(np.float32(128)))
+    hook = make_parity_hook(32, 8, 128, 16, 32, 50, 128, stats, scale)
+    report, log = trace_run.run_trace(trace, hook=hook, max_iters=400)
+    assert len(log) == 400 and len(stats) == 2 * 8 and {s[1] for s in stats} == {0, 31}
+    kw = dict(alpha=100.0, beta=-1.0, B_max=2048, S_max=1024, num_blocks=20480, block_size=16,
+              page_mb=2 * 8 * 16 * 128 * 2 * 32 / 2**20)
+    digest, n = replay_reference(trace, log, truncated=True, **kw)
+    assert n == 400 and digest == report["schedule_sha256"]
+    roof = report["attention_roofline_by_class"]
+    assert roof["all"]["algorithmic_bytes"] > 0 and 0 < roof["all"]["frac_of_hbm_peak"] < 1.2
+    os.makedirs("gpurun_out", exist_ok=True)
+    report["oracle_parity_samples"] = [{"iteration": s[0], "layer": s[1], "max_abs": s[2], "mean_abs": s[3]} for s in stats]
+    with open("gpurun_out/trace_config5_first400.json", "w") as f:
+        json.dump(report, f)
+
+
+def _lprs_loop(n_harvest, epochs, layers, n_requests, rate, max_iters, pages_per_layer, out_name):
+    """SURVEY.md 8(f) N1 on the N3 clock: harvest whole-forward-pass times (attention of every layer + dense GEMM
+    filler) through the serving loop's own IterationRunner, train the Table-7 MLP, take T* = the median time of the
+    full-budget rounds, then run the trace under token budget / LPRS / LPRS + APC with that predictor; every schedule
+    must equal the reference scheduler's replay on the measured times (same predictor data on both sides)."""
+    from paper_2606_09061_b200 import predictor as pr
+    build.build()
+    raw, us = pr.harvest(n_harvest, seed=0, layers=layers, layer_gemms=True, pages_per_layer=65536, repeats=2)
+    rep, lin, mlp = pr.train_and_report(raw, us, seed=0, epochs=epochs)
+    X = pr.features16(raw)
+    t_star = float(np.median(us[X[:, 12] >= 2000]))           # a typical full-budget round (PAPER.md:456: T* is a whole-iteration time)
+    trace = wl.make_trace(n_requests, rate_per_s=rate, seed=0)
+    kind, w, mu, inv = pr.export_mlp(mlp)
+    base = dict(alpha=100.0, beta=-1.0, B_max=2048, S_max=1024, num_blocks=pages_per_layer, block_size=16,
+                page_mb=2 * 8 * 16 * 128 * 2 * layers / 2**20)
+    lprs = dict(base, mode=rs.MODE_LPRS, Delta=64, T_star=t_star, lambda_u=1.0, lambda_o=2.0, C_max=4, L_min=64,
+                pred_kind=kind, pred_weights=w, feat_mu=mu, feat_inv_sigma=inv)
+    out = {"predictor": rep, "T_star_us": t_star, "arrival_rate_per_s": rate, "layers": layers,
+           "clock": "whole forward pass (attention + dense GEMM filler)", "runs": {}}
+    for name, kw in [("token_budget", base), ("lprs", lprs), ("lprs_apc", dict(lprs, apc=True))]:
+        report, log = trace_run.run_trace(trace, layers=layers, pages_per_layer=pages_per_layer, sched_kw=kw,
+                                          layer_gemms=True, max_iters=max_iters)
+        digest, n = replay_reference(trace, log, truncated=max_iters is not None, **kw)
+        assert n == len(log) and digest == report["schedule_sha256"], name
+        it = np.asarray(log, np.float64)
+        report["iteration_us"] = {"mean": float(it.mean()), "p50": float(np.percentile(it, 50)), "p95": float(np.percentile(it, 95)),
+                                  "p99": float(np.percentile(it, 99)), "max": float(it.max()), "frac_over_T_star": float((it > t_star).mean()),
+                                  "mean_abs_dev_from_T_star_of_mixed": None}
+        report.pop("sched", None)
+        out["runs"][name] = report
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(f"gpurun_out/{out_name}", "w") as f:
+        json.dump(out, f)
+    return out
+
+
+def test_lprs_apc_loop_on_the_whole_iteration_clock():
+    """Bounded version for every run: 300 harvested rounds, 30 epochs, a 4-layer model, 120 requests at 200 req/s, 500
+    iterations per mode.  Latency control ("minimizing deviation from a target latency budget"): LPRS
+    pulls the tail of the iteration time towards T*."""
+    out = _lprs_loop(300, 30, 4, 120, 200.0, 500, 20480, "lprs_report_bounded.json")
+    tb, lp = out["runs"]["token_budget"]["iteration_us"], out["runs"]["lprs"]["iteration_us"]
+    assert lp["p95"] <= tb["p95"] and lp["max"] <= tb["max"] * 1.05
+    assert out["predictor"]["mlp_test"]["mape_pct"] < 30.0
+
+
+@pytest.mark.skipif(os.environ.get("CP_FULL_TRACE") != "1", reason="set CP_FULL_TRACE=1 (long: 32 layers with GEMM filler)")
+def test_lprs_apc_loop_long():
+    out = _lprs_loop(int(os.environ.get("CP_HARVEST", "2500")), int(os.environ.get("CP_EPOCHS", "300")), 32, 1000,
+                     float(os.environ.get("CP_TRACE_RATE", "8")), None, 20480, "lprs_report.json")
+    assert out["predictor"]["mlp_test"]["mape_pct"] < 10.0
+
+
+def test_sharegpt_like_short_context_trace():
+    """the paper's short-context mix (prompt median 19, P90 179, max context 512,
+    generation <= 512) as a synthetic trace, in the compressed-arrival variant so that rounds carry many tiny chunks
+    (PAPER.md:488-497), aging scheduler with chunk budget 256 as in Table 4: oracle parity on sampled iterations,
+    schedule identity, and the per-iteration time against the small-batch floor."""
+    build.build()
+    Hq, Hkv, D, B, layers = 32, 8, 128, 16, 2
+    trace = wl.make_sharegpt_like_trace(200, gap_us=150.0, seed=6)
+    kw = dict(alpha=100.0, beta=-1.0, B_max=256, S_max=64, num_blocks=8192, block_size=B)
+    stats = []
+    scale = float(np.float32(1.0) / np.sqrt(np.float32(D)))
+    hook = make_parity_hook(Hq, Hkv, D, B, layers, 40, 192, stats, scale)
+    report, log = trace_run.run_trace(trace, Hq=Hq, Hkv=Hkv, D=D, B=B, layers=layers, pages_per_layer=8192,
+                                      sched_kw=kw, seed=6, hook=hook)
+    assert report["e2e_s"]["finished"] == 200 and len(stats) >= 10
+    digest, n = replay_reference(trace, log, **dict(kw, page_mb=2 * Hkv * B * D * 2 * layers / 2**20))
+    assert n == len(log) and digest == report["schedule_sha256"]
+    per_layer = np.asarray(log, np.float64) / layers
+    report["us_per_layer"] = {"p50": float(np.percentile(per_layer, 50)), "p95": float(np.percentile(per_layer, 95)), "min": float(per_layer.min())}
+    assert report["us_per_layer"]["p50"] < 60.0            # short contexts: a round is a few times the launch floor, not more
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/trace_sharegpt_like.json", "w") as f:
+        json.dump(report, f)
