@@ -25,26 +25,24 @@ __device__ __forceinline__ int64_t slab_elem_offset(int64_t page, int kv, int he
 // hold no key, and later appends overwrite them.  (K tails too: a K tile's stale rows can be left in a ring
 // slot that a shorter V tile later only partly overwrites.)  With that and the kernel's prologue clear, a
 // torch.empty pool or NaN-filled tails cannot reach a result (include/cp.h; reading R6).
-// One thread per 16-byte chunk of a (request, K|V, kv head, slot 1..15) row; most exit at once.
 // ---------------------------------------------------------------------------------
 __device__ __forceinline__ void zero_page_tails(const BatchMeta& meta, const Shape& sh, __nv_bfloat16* __restrict__ cache) {
-    const int chunks = sh.D / 8;
-    const int64_t total = (int64_t)meta.n_reqs * 2 * sh.Hkv * (sh.B - 1) * chunks;
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
-         i += (int64_t)gridDim.x * blockDim.x) {
-        const int c = (int)(i % chunks);
-        int64_t r = i / chunks;
-        const int slot = 1 + (int)(r % (sh.B - 1));
-        r /= (sh.B - 1);
-        const int g = (int)(r % sh.Hkv);
-        r /= sh.Hkv;
-        const int kv = (int)(r & 1);
-        const int req = (int)(r >> 1);
+    // one warp per (request, K|V, kv head) slab of the request's last page: the 32 lanes sweep the 16-byte chunks of
+    // the slots past the last key (contiguous memory: slots are adjacent rows of the slab)
+    const int lane = threadIdx.x & 31;
+    const int64_t n_warps = (int64_t)gridDim.x * (blockDim.x >> 5);
+    const int64_t total = (int64_t)meta.n_reqs * 2 * sh.Hkv;
+    for (int64_t w = blockIdx.x * (int64_t)(blockDim.x >> 5) + (threadIdx.x >> 5); w < total; w += n_warps) {
+        const int g = (int)(w % sh.Hkv);
+        const int kv = (int)((w / sh.Hkv) & 1);
+        const int req = (int)(w / (2 * sh.Hkv));
         const int last = meta.ctx_off[req] + meta.q_len[req] - 1;       // position of the request's last key
-        if (slot <= last % sh.B) continue;
+        const int first_free = last % sh.B + 1;
+        if (first_free >= sh.B) continue;
         const int64_t page = meta.block_table[meta.bt_off[req] + last / sh.B];
-        __nv_bfloat16* dst = cache + slab_elem_offset(page, kv, g, sh.Hkv, sh.B, sh.D) + (int64_t)slot * sh.D + c * 8;
-        *reinterpret_cast<uint4*>(dst) = make_uint4(0, 0, 0, 0);
+        uint4* dst = reinterpret_cast<uint4*>(cache + slab_elem_offset(page, kv, g, sh.Hkv, sh.B, sh.D) + (int64_t)first_free * sh.D);
+        const int n16 = (sh.B - first_free) * sh.D / 8;
+        for (int i = lane; i < n16; i += 32) dst[i] = make_uint4(0, 0, 0, 0);
     }
 }
 
@@ -200,24 +198,23 @@ __device__ __forceinline__ uint32_t e4m3x4(float a, float b, float c, float d) {
 
 __device__ __forceinline__ void zero_page_tails8(const BatchMeta& meta, const Shape& sh, uint8_t* __restrict__ cache8,
                                                  float* __restrict__ scales) {
-    const int chunks = sh.D / 16;                                 // 16-byte chunks per row of codes
-    const int64_t total = (int64_t)meta.n_reqs * 2 * sh.Hkv * (sh.B - 1) * chunks;
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
-         i += (int64_t)gridDim.x * blockDim.x) {
-        const int c = (int)(i % chunks);
-        int64_t r = i / chunks;
-        const int slot = 1 + (int)(r % (sh.B - 1));
-        r /= (sh.B - 1);
-        const int g = (int)(r % sh.Hkv);
-        r /= sh.Hkv;
-        const int kv = (int)(r & 1);
-        const int req = (int)(r >> 1);
+    // one warp per (request, K|V, kv head) slab of the request's last page, as zero_page_tails
+    const int lane = threadIdx.x & 31;
+    const int64_t n_warps = (int64_t)gridDim.x * (blockDim.x >> 5);
+    const int64_t total = (int64_t)meta.n_reqs * 2 * sh.Hkv;
+    for (int64_t w = blockIdx.x * (int64_t)(blockDim.x >> 5) + (threadIdx.x >> 5); w < total; w += n_warps) {
+        const int g = (int)(w % sh.Hkv);
+        const int kv = (int)((w / sh.Hkv) & 1);
+        const int req = (int)(w / (2 * sh.Hkv));
         const int last = meta.ctx_off[req] + meta.q_len[req] - 1;
-        if (slot <= last % sh.B) continue;
+        const int first_free = last % sh.B + 1;
+        if (first_free >= sh.B) continue;
         const int64_t page = meta.block_table[meta.bt_off[req] + last / sh.B];
-        const int64_t row = slab8_offset(page, kv, g, sh.Hkv, sh.B) + slot;
-        *reinterpret_cast<uint4*>(cache8 + row * sh.D + c * 16) = make_uint4(0, 0, 0, 0);
-        if (c == 0) scales[row] = 1.f;
+        const int64_t row0 = slab8_offset(page, kv, g, sh.Hkv, sh.B) + first_free;
+        uint4* dst = reinterpret_cast<uint4*>(cache8 + row0 * sh.D);
+        const int n16 = (sh.B - first_free) * sh.D / 16;
+        for (int i = lane; i < n16; i += 32) dst[i] = make_uint4(0, 0, 0, 0);
+        if (lane < sh.B - first_free) scales[row0 + lane] = 1.f;
     }
 }
 

@@ -194,6 +194,18 @@ def test_latency_table_rows():
     assert list(r.feat) == [48.0, 2.0, 4.0, 140.0, 100.0, 48.0, 48.0, 10.0, 20.0, 5.0, 8.0]
     assert (r.n_prefill, r.n_decode, r.iter) == (2, 2, 0)
     assert ctx.cp_latency_table() == []
+    # a 1-token prefill chunk (Eq. 8's candidate c = 1, the last token of a prompt) is flagged by the scheduler and
+    # counts as prefill in the Table-1 features, as in the scheduler's own feature vector; unflagged it is a decode
+    ctx.cp_build_batch([1, 1], [7, 99], [spec.block_tables[0], spec.block_tables[3]], flags=[binding.CP_REQ_PREFILL, 0])
+    ctx.cp_attention_step(0, gu.torch_bf16(hv.q[:2]), None, None, pool, out)
+    r = ctx.cp_latency_table()[0]
+    assert list(r.feat[:7]) == [1.0, 1.0, 2.0, 100.0, 100.0, 7.0, 7.0] and (r.n_prefill, r.n_decode) == (1, 1)
+    # all layers in one submission: one row for the iteration, layer = -n
+    pa = binding.Context.pointer_array
+    q2 = gu.torch_bf16(hv.q[:2])
+    ctx.cp_attention_layers(pa([q2] * 3), None, None, pa([pool] * 3), pa([out] * 3))
+    rows = ctx.cp_latency_table()
+    assert len(rows) == 1 and rows[0].layer == -3 and rows[0].us > 0
     ctx.close()
 
 
