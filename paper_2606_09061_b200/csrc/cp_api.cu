@@ -676,7 +676,7 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const 
         // batches run chunk tiles and decode streams side by side (dual lane); tensor-bound batches put both softmax
         // warpgroups on every chunk tile (SPLIT) and move a quarter of the exponentials to the FMA pipe.
         if (c->tensor_bound)
-            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, true, true, false>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, true>::kTotal, stream, p, tmap_copy, *tmap8));
+            CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, true, true, false>, dim3(grid), dim3(dl::kThreadsSplit), dl::Layout<D, true>::kTotal, stream, p, tmap_copy, *tmap8));
         else
             CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, false, false, false>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, false>::kTotal, stream, p, tmap_copy, *tmap8));
         CP_CUDA(cudaGetLastError());

@@ -54,6 +54,19 @@ namespace cp {
 namespace dl {
 
 constexpr int kThreads = 512;
+// SPLIT mode: kSplitWG softmax warpgroups share every chunk tile (each thread <-> a row and 128 / kSplitWG of its
+// keys).  Two (512 threads) is the measured optimum on B200: four (768 threads, 96 registers per softmax thread,
+// 32 keys per thread) runs the chunk-only batch in 361 us against 331 us and the 70B-shaped batch in 37.8 ms
+// against 34.7 ms -- the per-tile fixed cost of a warp (barrier waits, TMEM round trips, the maximum exchange)
+// is paid by twice as many warps in lockstep.
+#ifndef DL_SPLIT_WG
+#define DL_SPLIT_WG 2
+#endif
+constexpr int kSplitWG = DL_SPLIT_WG;
+static_assert(kSplitWG == 2 || kSplitWG == 4, "SPLIT: two or four softmax warpgroups");
+constexpr int kSplitCols = 128 / kSplitWG;           // keys of a tile per softmax thread
+constexpr int kThreadsSplit = 256 + 128 * kSplitWG;
+template <bool SPLIT> __host__ __device__ constexpr int threads_of() { return SPLIT ? kThreadsSplit : kThreads; }
 constexpr int kStagesT = 3, kStagesS = 3, kMaxStages = 6;
 constexpr int kStagesSplit = 6, kProdSplit = 5;  // SPLIT mode: one ring, all five producer warps
 constexpr int kStagesS8 = 6;                     // fp8 pools: lane S's ring is six 16 KiB slots (same bytes in flight)
@@ -368,8 +381,8 @@ __device__ __forceinline__ void mma_tile_item(const WorkItem& it, uint32_t smem_
 }
 
 // SPLIT mode, tile kind (one issuer warp): per 128-key tile t one score block QK(t) -- TS form, Q in TMEM, N = 128
-// keys, into S buffer (tile counter & 1) -- and one PV block over the whole tile once BOTH softmax warpgroups have
-// delivered their half of P(t) (tp_full counts their eight warps).  QK(t+1) is issued ahead of PV(t), so the next
+// keys, into S buffer (tile counter & 1) -- and one PV block over the whole tile once ALL softmax warpgroups have
+// delivered their part of P(t) (tp_full counts their warps).  QK(t+1) is issued ahead of PV(t), so the next
 // scores wait for the warpgroups while the pipe runs PV(t); it overwrites the buffer PV(t-1) read: same thread,
 // program order, in-order pipe -- no barrier.  K-steps (pages) past the item's last key are not multiplied.
 template <int D>
@@ -417,9 +430,10 @@ __device__ __forceinline__ void mma_split_item(const WorkItem& it, uint32_t smem
 #pragma unroll
             for (int ks = 0; ks < kKeyTile / 16; ++ks) {
                 // V (MN-major): 16 key rows = 2 row groups (SBO apart); the next 64 d are 1 KB further (LBO).
-                // P of keys 64 w .. 64 w + 63 sits in the first 32 columns of half w of the S buffer.
+                // P of keys kSplitCols w .. kSplitCols (w + 1) - 1 sits in the first kSplitCols / 2 columns of
+                // part w of the S buffer.
                 if (t * kKeyTile + ks * 16 < n_keys)
-                    umma_ts(tmem + col_o(0), tmem + buf * 128 + (ks >> 2) * 64 + (ks & 3) * 8,
+                    umma_ts(tmem + col_o(0), tmem + buf * 128 + (ks * 16 / kSplitCols) * kSplitCols + (ks * 16 % kSplitCols) / 2,
                             ptx::umma_desc_advance(v_desc0, ks * L::kPageBytes), idesc_pv, t > 0 || ks > 0);
             }
             ptx::umma_commit(&ls->kv_empty[slot]);
@@ -765,17 +779,21 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
 }
 
 // ------------------------------------------------------------------------------------------
-// SPLIT mode: softmax of warpgroup w (0 / 1) for a chunk tile: thread <-> row of the 128-row Q tile, columns
-// (keys) [64 w, 64 w + 64) of every 128-key score tile.  Per tile: the half score row from TMEM, its maximum,
-// the exchange of the two half-row maxima through shared memory (one 256-thread named barrier), then both
-// threads of a row take the SAME decision about the reference maximum (lazy rescale: only when the row maximum
-// grew by more than 2^8), exponentials, partial row sum of the own columns, P (bf16 pairs) back over the scores
-// of the own half.  Warpgroup w owns O columns [w D/2, (w + 1) D/2) for the rescale and the epilogue; the two
-// partial row sums meet in shared memory at the end.  Warpgroup 0 puts the Q tile into TMEM.
+// SPLIT mode: softmax of warpgroup w (0 .. kSplitWG - 1) for a chunk tile: thread <-> row of the 128-row Q tile,
+// columns (keys) [kSplitCols w, kSplitCols (w + 1)) of every 128-key score tile.  Per tile: the part of the score
+// row from TMEM, its maximum, the exchange of the part-row maxima through shared memory (one named barrier over
+// the kSplitWG warps that hold the same 32 rows), then all threads of a row take the SAME decision about the
+// reference maximum (lazy rescale: only when the row maximum grew by more than 2^8), exponentials, partial row sum
+// of the own columns, P (bf16 pairs) back over the scores of the own part.  Warpgroup w owns O columns
+// [w D / kSplitWG, (w + 1) D / kSplitWG) for the rescale and the epilogue; the partial row sums meet in shared
+// memory at the end.  Warpgroup 0 puts the Q tile into TMEM.
 // ------------------------------------------------------------------------------------------
 template <int D, bool POLY>
 __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& p, LaneState* ls, uint32_t tmem, uint8_t* xchg,
                                               uint32_t& gt, int row, uint32_t lane_base, int w) {
+    constexpr int NW = kSplitWG, CW = kSplitCols;        // warpgroups; keys of a tile per thread
+    constexpr int OC = D / NW;                           // O columns per warpgroup
+    constexpr int CH = OC < 32 ? OC : 32;                // ... handled CH at a time
     const Shape& sh = p.sh;
     const int G = sh.G;
     const int gs = 31 - __clz(G);                        // G is a power of two (cp_create): shifts, not divisions
@@ -788,9 +806,11 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
     const int head = it.kv_head * G + (row & (G - 1));
     const float scale = sh.sm_scale * 1.4426950408889634f;
     const uint32_t t_row = tmem + (lane_base << 16);
-    const uint32_t c_o = col_o(0) + w * (D / 2);         // this warpgroup's half of the O columns
-    float* xmax = reinterpret_cast<float*>(xchg);        // [tile parity][warpgroup][row]: half-row maxima (raw scores)
-    float* xl = xmax + 512;                              // [warpgroup][row]: partial row sums
+    const uint32_t c_o = col_o(0) + w * OC;              // this warpgroup's part of the O columns
+    float* xmax = reinterpret_cast<float*>(xchg);        // [tile parity][warpgroup][row]: part-row maxima (raw scores)
+    float* xl = xmax + 2 * NW * 128;                     // [warpgroup][row]: partial row sums
+    const int bar_id = 3 + (int)(lane_base >> 5);        // the NW warps that hold the same 32 rows
+    constexpr int bar_n = 32 * NW;
 
     if (w == 0) {
         // ---- Q row -> TMEM (A operand of QK^T): column j holds elements (2j, 2j+1)
@@ -814,28 +834,32 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
     float m_ref = -INFINITY, l = 0.f;
 
     for (int t = 0; t < n_tiles; ++t) {
-        const int ts = it.kv_begin + t * kKeyTile + w * 64;
+        const int ts = it.kv_begin + t * kKeyTile + w * CW;
         const uint32_t buf = gt & 1;
-        const uint32_t t_s = t_row + buf * 128 + w * 64;
+        const uint32_t t_s = t_row + buf * 128 + w * CW;
         ptx::mbar_wait(&ls->ts_full[buf], (gt >> 1) & 1);
         ptx::tc_fence_after();
-        uint32_t sr[64];
-        ptx::tmem_ld32(t_s, sr);
-        ptx::tmem_ld32(t_s + 32, sr + 32);
-        ptx::tmem_wait_ld();
-        const int nvalid = max(0, min(64, limit - ts));
-        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};      // independent max chains
-        if (nvalid == 64) {
+        uint32_t sr[CW];
 #pragma unroll
-            for (int i = 0; i < 64; ++i) mx[i & 3] = fmaxf(mx[i & 3], __uint_as_float(sr[i]));
+        for (int c = 0; c < CW / 32; ++c) ptx::tmem_ld32(t_s + c * 32, sr + c * 32);
+        ptx::tmem_wait_ld();
+        const int nvalid = max(0, min(CW, limit - ts));
+        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};      // independent max chains
+        if (nvalid == CW) {
+#pragma unroll
+            for (int i = 0; i < CW; ++i) mx[i & 3] = fmaxf(mx[i & 3], __uint_as_float(sr[i]));
         } else {
 #pragma unroll
-            for (int i = 0; i < 64; ++i) mx[i & 3] = fmaxf(mx[i & 3], i < nvalid ? __uint_as_float(sr[i]) : -INFINITY);
+            for (int i = 0; i < CW; ++i) mx[i & 3] = fmaxf(mx[i & 3], i < nvalid ? __uint_as_float(sr[i]) : -INFINITY);
         }
         const float m_loc = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
-        xmax[(gt & 1) * 256 + w * 128 + row] = m_loc;
-        ptx::named_bar_sync(3 + (int)(lane_base >> 5), 64);   // this warp and its partner (same rows, other half): its maxima are there
-        const float m_t = fmaxf(m_loc, xmax[(gt & 1) * 256 + (w ^ 1) * 128 + row]) * scale;     // scale > 0
+        float* xm = xmax + (gt & 1) * NW * 128 + row;
+        xm[w * 128] = m_loc;
+        ptx::named_bar_sync(bar_id, bar_n);               // the warps of the other warpgroups with the same rows: their maxima are there
+        float m_all = m_loc;
+#pragma unroll
+        for (int k = 1; k < NW; ++k) m_all = fmaxf(m_all, xm[((w + k) & (NW - 1)) * 128]);
+        const float m_t = m_all * scale;                  // scale > 0
         float alpha = 1.f;
         bool rescale = false;
         if (m_t > m_ref + kRescaleThreshold) {          // also the first finite max (m_ref = -inf)
@@ -845,38 +869,45 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
         }
         const float neg_m = (m_ref == -INFINITY) ? 0.f : -m_ref;
         float sm[4] = {0.f, 0.f, 0.f, 0.f};             // independent sum chains
-        uint32_t pk[32];                                // 64 scores -> 32 packed P columns
-        if (nvalid == 64) {
+        uint32_t pk[CW / 2];                            // CW scores -> CW / 2 packed P columns
+        if (nvalid == CW) {
+            // two columns per instruction (FFMA2 / FADD2); every kPolyEvery-th PAIR takes the FMA-pipe exponential
+            const float2 sc2 = make_float2(scale, scale), nm2 = make_float2(neg_m, neg_m);
+            float2 s2[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
-            for (int i = 0; i < 64; i += 2) {
-                const float a = ex2_sel<POLY>(fmaf(__uint_as_float(sr[i]), scale, neg_m), i);
-                const float b = ex2_sel<POLY>(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1);
-                sm[(i >> 1) & 3] += a + b;
-                pk[i >> 1] = pack_bf16(a, b);
+            for (int j = 0; j < CW / 2; ++j) {
+                const float2 x = ptx::fma2(make_float2(__uint_as_float(sr[2 * j]), __uint_as_float(sr[2 * j + 1])), sc2, nm2);
+                float2 e;
+                if (POLY && kPolyEvery > 0 && j % (kPolyEvery > 0 ? kPolyEvery : 1) == (kPolyEvery > 0 ? kPolyEvery : 1) - 1) e = ptx::ex2_poly2(x);
+                else e = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));
+                s2[j & 3] = ptx::add2(s2[j & 3], e);
+                pk[j] = pack_bf16(e.x, e.y);
             }
+            const float2 s01 = ptx::add2(ptx::add2(s2[0], s2[1]), ptx::add2(s2[2], s2[3]));
+            sm[0] = s01.x + s01.y;
         } else {
 #pragma unroll
-            for (int i = 0; i < 64; i += 2) {
+            for (int i = 0; i < CW; i += 2) {
                 const float a = i < nvalid ? ex2_sel<POLY>(fmaf(__uint_as_float(sr[i]), scale, neg_m), i) : 0.f;
                 const float b = i + 1 < nvalid ? ex2_sel<POLY>(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1) : 0.f;
                 sm[(i >> 1) & 3] += a + b;
                 pk[i >> 1] = pack_bf16(a, b);
             }
         }
-        ptx::tmem_st32(t_s, pk);
+        ptx::tmem_st<CW / 2>(t_s, pk);
         l = l * alpha + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
-        // same rows, same m_t, same m_ref in warp k of both warpgroups: the same decision on both sides
+        // same rows, same m_t, same m_ref in warp k of every warpgroup: the same decision on all sides
         if (t > 0 && __any_sync(0xffffffffu, rescale)) {
             ptx::mbar_wait(&ls->tpv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);      // PV(t-1) (and all before) done: O readable
             ptx::tc_fence_after();
 #pragma unroll 1
-            for (int c = 0; c < D / 64; ++c) {
-                uint32_t o[32];
-                ptx::tmem_ld32(t_row + c_o + c * 32, o);
+            for (int c = 0; c < OC / CH; ++c) {
+                uint32_t o[CH];
+                ptx::tmem_ld<CH>(t_row + c_o + c * CH, o);
                 ptx::tmem_wait_ld();
 #pragma unroll
-                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-                ptx::tmem_st32(t_row + c_o + c * 32, o);
+                for (int i = 0; i < CH; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                ptx::tmem_st<CH>(t_row + c_o + c * CH, o);
             }
         }
         ptx::tmem_wait_st();
@@ -885,24 +916,27 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
         ++gt;
     }
 
-    // ---- epilogue: this warpgroup's half of the O row -> out (bf16, normalised) or split workspace (fp32, unnormalised)
+    // ---- epilogue: this warpgroup's part of the O row -> out (bf16, normalised) or split workspace (fp32, unnormalised)
     ptx::mbar_wait(&ls->tpv_done[(gt - 1) & 1], ((gt - 1) >> 1) & 1);
     ptx::tc_fence_after();
     xl[w * 128 + row] = l;
-    ptx::named_bar_sync(3 + (int)(lane_base >> 5), 64);
-    l += xl[(w ^ 1) * 128 + row];
+    ptx::named_bar_sync(bar_id, bar_n);
+    // every warpgroup adds the partial sums in the same order: the same l on all sides
+    l = 0.f;
+#pragma unroll
+    for (int k = 0; k < NW; ++k) l += xl[k * 128 + row];
     const float inv = 1.f / l;
 #pragma unroll 1
-    for (int c = 0; c < D / 64; ++c) {
-        uint32_t o[32];
-        ptx::tmem_ld32(t_row + c_o + c * 32, o);
+    for (int c = 0; c < OC / CH; ++c) {
+        uint32_t o[CH];
+        ptx::tmem_ld<CH>(t_row + c_o + c * CH, o);
         ptx::tmem_wait_ld();
         if (!valid_row) continue;
-        const int d0 = w * (D / 2) + c * 32;
+        const int d0 = w * OC + c * CH;
         if (it.partial_row < 0) {
             uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * sh.Hq + head) * D + d0);
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+            for (int j = 0; j < CH / 8; ++j)
                 dst[j] = make_uint4(pack_bf16(__uint_as_float(o[8 * j]) * inv, __uint_as_float(o[8 * j + 1]) * inv),
                                     pack_bf16(__uint_as_float(o[8 * j + 2]) * inv, __uint_as_float(o[8 * j + 3]) * inv),
                                     pack_bf16(__uint_as_float(o[8 * j + 4]) * inv, __uint_as_float(o[8 * j + 5]) * inv),
@@ -910,12 +944,12 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
         } else {
             uint4* dst = reinterpret_cast<uint4*>(p.part_o + ((int64_t)it.partial_row + row) * D + d0);
 #pragma unroll
-            for (int j = 0; j < 8; ++j) dst[j] = make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+            for (int j = 0; j < CH / 4; ++j) dst[j] = make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
         }
     }
     if (w == 0 && valid_row && it.partial_row >= 0) p.part_ml[(int64_t)it.partial_row + row] = make_float2(m_ref, l);
     ptx::tc_fence_before();
-    ptx::named_bar_sync(3 + (int)(lane_base >> 5), 64);  // the exchange arrays are reused by the next item
+    ptx::named_bar_sync(bar_id, bar_n);                  // the exchange arrays are reused by the next item
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1267,10 +1301,10 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
 
 // softmax warpgroup loop.  ROLE 0: lane T (tile kind, and the swap-kind items lane T picks up);
 // ROLE 2: lane S.
-// SPLIT: both warpgroups follow lane 0's item ring; ROLE 0 = warpgroup 0 of the column split (and the swap-kind
-// items), ROLE 2 = warpgroup 1 (swap-kind items are skipped).
+// SPLIT: all warpgroups follow lane 0's item ring; ROLE 0 = warpgroup 0 of the column split (and the swap-kind
+// items), ROLE 2 = warpgroups wg >= 1 (swap-kind items are skipped).
 template <int D, int ROLE, bool POLY, bool SPLIT, bool KV8>
-__device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Misc* misc, int warp, int lane) {
+__device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Misc* misc, int warp, int lane, int wg = 0) {
     using L = Layout<D, SPLIT>;
     constexpr int LANE = (ROLE == 2 && !SPLIT) ? 1 : 0;
     LaneState* ls = &misc->lane[LANE];
@@ -1287,7 +1321,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
         if (it.kind < 0) break;
         if constexpr (SPLIT) {
             if (it.kind == kKindTile) {
-                softmax_split<D, POLY>(it, p, ls, tmem, small, gh_tile, row, lane_base, ROLE == 2 ? 1 : 0);
+                softmax_split<D, POLY>(it, p, ls, tmem, small, gh_tile, row, lane_base, ROLE == 2 ? wg : 0);
                 ++item_cnt;
                 continue;
             }
@@ -1317,7 +1351,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
 // KV8 (fp8 pools, dual-lane only): tmap = the library's bf16 scratch pool (chunk tiles), tmap8 = the e4m3 pool (decode
 // streams); otherwise tmap = the bf16 pool and tmap8 is a copy of it, unused.
 template <int D, bool POLY, bool SPLIT, bool KV8>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(threads_of<SPLIT>(), 1)
 attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap8) {
     static_assert(!(KV8 && (SPLIT || D != 128)), "fp8 pools: dual-lane instantiation, D = 128");
     using L = Layout<D, SPLIT>;
@@ -1340,13 +1374,13 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap, const _
             }
             for (int i = 0; i < 4; ++i) {
                 ptx::mbar_init(&ls->ts_full[i], 1);
-                ptx::mbar_init(&ls->tp_full[i], SPLIT ? 8 : 4);      // SPLIT: both warpgroups deliver a half of P
+                ptx::mbar_init(&ls->tp_full[i], SPLIT ? 4 * kSplitWG : 4);      // SPLIT: every warpgroup delivers its part of P
                 ptx::mbar_init(&ls->tpv_done[i], 1);
                 ptx::mbar_init(&ls->pv_issued[i], 1);
             }
             // readers of the item ring (one arrival per warp): the lane's 4 softmax warps, its MMA warp(s), its other producers
-            // (SPLIT: one ring for everybody -- 8 softmax warps, 1 issuer, the other producers)
-            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], SPLIT ? 8 + 1 + kProdSplit - 1 : 4 + (ln == 0 ? 2 + kProdT - 1 : 1 + kProdS - 1)); }
+            // (SPLIT: one ring for everybody -- the softmax warps, 1 issuer, the other producers)
+            for (int i = 0; i < kItemRing; ++i) { ptx::mbar_init(&ls->item_full[i], 1); ptx::mbar_init(&ls->item_empty[i], SPLIT ? 4 * kSplitWG + 1 + kProdSplit - 1 : 4 + (ln == 0 ? 2 + kProdT - 1 : 1 + kProdS - 1)); }
         }
         ptx::fence_barrier_init();
         ptx::prefetch_tmap(&tmap);
@@ -1357,7 +1391,7 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap, const _
     // masked P = 0 times a NaN V row would poison the accumulators.  After this clear everything that ever sits
     // in the ring is finite: K/V rows that are keys of their request, page tails that the append kernel zeroed
     // (cp_kernels_simt.cuh), or these zeros.
-    for (uint32_t i = threadIdx.x * 16; i < L::kOffMisc; i += kThreads * 16)
+    for (uint32_t i = threadIdx.x * 16; i < L::kOffMisc; i += threads_of<SPLIT>() * 16)
         *reinterpret_cast<uint4*>(smem + i) = make_uint4(0, 0, 0, 0);
     ptx::fence_proxy_async_smem();
     ptx::tc_fence_before();
@@ -1367,21 +1401,23 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap, const _
     ptx::grid_dep_wait();
     ptx::grid_dep_launch();                              // the combine kernel may stage its launch
 
-    // launch allocation: 128 registers per thread.  The two producer / MMA warpgroups give most of
-    // their share to the tile softmax (a 128-column score row in registers) and the decode softmax.
+    // launch allocation: 128 registers per thread (SPLIT with four warpgroups: 768 threads at 80).  The two
+    // producer / MMA warpgroups give most of their share to the tile softmax (a score row, or its part, in
+    // registers) and the decode softmax.
+    constexpr bool kWide = SPLIT && kSplitWG == 4;       // 8 warps x 48 + 16 warps x 96 = 24 warps x 80
     if (warp < 8) {
-        reg_dec<56>();
+        reg_dec<kWide ? 48 : 56>();
         if (warp < kProdT + kProdS) producer<D, SPLIT, KV8>(p, &tmap, &tmap8, smem, misc, lane, warp);
         else if (warp == 5) mma_warp<D, 0, 1, SPLIT, KV8>(ptx::smem_u32(smem), misc, lane);     // lane T: score blocks (and swap items); SPLIT: the one issuer
         else if (SPLIT) { }                                                                      // SPLIT: warps 6, 7 have no role
         else if (warp == 6) mma_warp<D, 0, 2, false, KV8>(ptx::smem_u32(smem), misc, lane);     // lane T: PV blocks
         else mma_warp<D, 1, 0, false, KV8>(ptx::smem_u32(smem), misc, lane);                    // lane S
     } else if (warp < 12) {
-        reg_inc<SPLIT ? 200 : 232>();
+        reg_inc<kWide ? 96 : SPLIT ? 200 : 232>();
         softmax_warps<D, 0, POLY, SPLIT, KV8>(p, smem, misc, warp, lane);
     } else {
-        reg_inc<SPLIT ? 200 : 160>();
-        softmax_warps<D, 2, SPLIT && POLY, SPLIT, KV8>(p, smem, misc, warp, lane);
+        reg_inc<kWide ? 96 : SPLIT ? 200 : 160>();
+        softmax_warps<D, 2, SPLIT && POLY, SPLIT, KV8>(p, smem, misc, warp, lane, (warp - 8) >> 2);
     }
     ptx::tc_fence_before();
     __syncthreads();

@@ -195,9 +195,11 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
 template <> __device__ __forceinline__ void tmem_ld<4>(uint32_t a, uint32_t* r) { tmem_ld4(a, r); }
 template <> __device__ __forceinline__ void tmem_ld<8>(uint32_t a, uint32_t* r) { tmem_ld8(a, r); }
 template <> __device__ __forceinline__ void tmem_ld<16>(uint32_t a, uint32_t* r) { tmem_ld16(a, r); }
+template <> __device__ __forceinline__ void tmem_ld<32>(uint32_t a, uint32_t* r) { tmem_ld32(a, r); }
 template <> __device__ __forceinline__ void tmem_st<4>(uint32_t a, const uint32_t* r) { tmem_st4(a, r); }
 template <> __device__ __forceinline__ void tmem_st<8>(uint32_t a, const uint32_t* r) { tmem_st8(a, r); }
 template <> __device__ __forceinline__ void tmem_st<16>(uint32_t a, const uint32_t* r) { tmem_st16(a, r); }
+template <> __device__ __forceinline__ void tmem_st<32>(uint32_t a, const uint32_t* r) { tmem_st32(a, r); }
 
 // order-preserving float <-> int map (an involution), so a float max is one REDUX.MAX.S32
 __device__ __forceinline__ int f2ord(float f) {
@@ -285,6 +287,32 @@ __device__ __forceinline__ float ex2_poly(float x) {
     p = fmaf(p, f, 0.69326097f);
     p = fmaf(p, f, 0.99992806f);
     return __int_as_float(__float_as_int(p) + (__float_as_int(xr) << 23));
+}
+// Packed fp32 pairs (sm_100: FFMA2 / FADD2): two lanes per instruction, each lane IEEE round-to-nearest like the
+// scalar form -- the same values in half the issue slots.
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    uint64_t rd;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd)
+        : "l"(*reinterpret_cast<uint64_t*>(&a)), "l"(*reinterpret_cast<uint64_t*>(&b)), "l"(*reinterpret_cast<uint64_t*>(&c)));
+    return *reinterpret_cast<float2*>(&rd);
+}
+__device__ __forceinline__ float2 add2(float2 a, float2 b) {
+    uint64_t rd;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(*reinterpret_cast<uint64_t*>(&a)), "l"(*reinterpret_cast<uint64_t*>(&b)));
+    return *reinterpret_cast<float2*>(&rd);
+}
+// ex2_poly on a pair: the same steps and constants per lane
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+    x.x = fmaxf(x.x, -126.f);
+    x.y = fmaxf(x.y, -126.f);
+    const float2 big = make_float2(12582912.f, 12582912.f), nbig = make_float2(-12582912.f, -12582912.f);
+    const float2 xr = add2(x, big);
+    const float2 f = fma2(add2(xr, nbig), make_float2(-1.f, -1.f), x);      // x - round(x)
+    float2 p = fma2(make_float2(0.05517165f, 0.05517165f), f, make_float2(0.24261113f, 0.24261113f));
+    p = fma2(p, f, make_float2(0.69326097f, 0.69326097f));
+    p = fma2(p, f, make_float2(0.99992806f, 0.99992806f));
+    return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
+                       __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
 }
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;
