@@ -714,13 +714,20 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
         float sm[4] = {0.f, 0.f, 0.f, 0.f};             // independent sum chains
         uint32_t pk[32];                                // 64 scores -> 32 packed P columns
         if (nvalid == 64) {
+            // two columns per instruction (FFMA2 / FADD2), as in softmax_split
+            const float2 sc2 = make_float2(scale, scale), nm2 = make_float2(neg_m, neg_m);
+            float2 s2[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
-            for (int i = 0; i < 64; i += 2) {
-                const float a = ex2_sel<POLY>(fmaf(__uint_as_float(sr[i]), scale, neg_m), i);
-                const float b = ex2_sel<POLY>(fmaf(__uint_as_float(sr[i + 1]), scale, neg_m), i + 1);
-                sm[(i >> 1) & 3] += a + b;
-                pk[i >> 1] = pack_bf16(a, b);
+            for (int i = 0; i < 32; ++i) {
+                const float2 x = ptx::fma2(make_float2(__uint_as_float(sr[2 * i]), __uint_as_float(sr[2 * i + 1])), sc2, nm2);
+                float2 e;
+                if (POLY && kPolyEvery > 0 && i % (kPolyEvery > 0 ? kPolyEvery : 1) == (kPolyEvery > 0 ? kPolyEvery : 1) - 1) e = ptx::ex2_poly2(x);
+                else e = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));
+                s2[i & 3] = ptx::add2(s2[i & 3], e);
+                pk[i] = pack_bf16(e.x, e.y);
             }
+            const float2 s01 = ptx::add2(ptx::add2(s2[0], s2[1]), ptx::add2(s2[2], s2[3]));
+            sm[0] = s01.x + s01.y;
         } else {
 #pragma unroll
             for (int i = 0; i < 64; i += 2) {
