@@ -361,6 +361,9 @@ def run_ours(args):
                      "t_hbm_us": t_hbm * 1e6, "t_tensor_us": t_tc * 1e6,
                      "frac_nominal_8TBs_2250TF": max(bytes_alg / 8e12, flops_alg / 2.25e15) / (attn_us * 1e-6)},
     }
+    if bound == "hbm" and achieved > peak:
+        # the peak is a COPY (half reads, half writes); a read-only stream runs above it on this part
+        res["roofline"]["note"] = "achieved > peak: the measured peak is a read+write copy, this batch is a read-only stream"
     if world == 1 and not args.no_cpu_baseline and not fp8:
         from oracle import attention as ora
         cache = compact.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
