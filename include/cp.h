@@ -297,6 +297,38 @@ int cp_sched_select_chunk(cp_sched* s, int32_t r_i, int32_t ctx_i, int32_t U_t,
                           int32_t pf_tokens, int32_t n_pf, int64_t pf_proc,
                           int32_t pf_proc_max, int32_t* c_star);
 
+/* ---- an entry point that allocates nothing ---------------------------------------------------------------------
+ * cp_decode_attention_static: split-KV decode attention (q_len = 1 per request) over a bf16 paged KV pool, for
+ * callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it).  It needs no cp_ctx and calls no cudaMalloc / cudaFree / allocating library routine: the split-KV partials
+ * (one unnormalised fp32 O row and one (m, l) pair per (request, q head, split)) live in a file-scope static device
+ * array of CP_STATIC_SCRATCH_BYTES (about 2 MiB) inside libcp.so, which every GPU that loads the library holds until
+ * the process exits.  Operation: the same as cp_attention_step for a decode:
+ * row (request j, q head h) attends to keys [0, kv_len[j]) of KV head h / (num_q_heads / num_kv_heads); fp32
+ * softmax, bf16 out.  Plain-ALU kernels (one warp per partial row): a convenience path, not the tuned one.
+ *
+ *   q             DEVICE  bf16 [n_reqs][num_q_heads][head_dim]
+ *   kv_cache      DEVICE  bf16 [num_blocks][2][num_kv_heads][block_size][head_dim]   (the layout of cp_attention_step;
+ *                 the new token's K/V row must already be in its page: this call appends nothing)
+ *   block_tables  DEVICE  int32 [n_reqs][max_pages_per_req]; row j holds the pages of request j, entries past
+ *                 ceil(kv_len[j] / block_size) are not read
+ *   kv_len        DEVICE  int32 [n_reqs], each >= 1 (keys of the request, the new token included)
+ *   n_splits      key-range splits per row, >= 1 (more splits = more parallelism for few long requests)
+ *   out           DEVICE  bf16 [n_reqs][num_q_heads][head_dim]
+ *   stream        cudaStream_t (NULL = default stream); the call only enqueues two kernels on it
+ * Nothing is owned or kept by the library.  kv_len and the page ids are on the device and are NOT checked.
+ * Limit: n_reqs * num_q_heads * n_splits <= CP_STATIC_MAX_PARTIAL_ROWS, else CP_ECAPACITY (nothing is launched);
+ * head_dim 64 or 128.  Other errors: CP_EINVAL (null pointer, bad shape), CP_ECUDA.
+ * The array is shared by ALL calls on a device and keeps the last call's contents.  Every call overwrites each
+ * partial it later reads, so nothing needs clearing between calls; but calls that overlap on the GPU (different
+ * streams, or several host threads on one device) race on it: serialise them on one stream. */
+#define CP_STATIC_MAX_PARTIAL_ROWS 4096
+#define CP_STATIC_SCRATCH_BYTES    (CP_STATIC_MAX_PARTIAL_ROWS * (128 * 4 + 8))
+int cp_decode_attention_static(const void* q, const void* kv_cache, const int32_t* block_tables,
+                               const int32_t* kv_len, int32_t n_reqs, int32_t max_pages_per_req,
+                               int32_t num_q_heads, int32_t num_kv_heads, int32_t head_dim,
+                               int32_t block_size, float sm_scale, int32_t n_splits, void* out, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -29,6 +29,7 @@ EXPORTS = [
     "cp_sched_next_arrival", "cp_sched_has_work", "cp_sched_get_stats",
     "cp_sched_request_times", "cp_sched_predict", "cp_sched_select_chunk",
     "cp_enable_rope", "cp_attention_step_rope", "cp_attention_step_fp8", "cp_attention_layers",
+    "cp_decode_attention_static",
 ]
 
 
@@ -129,6 +130,7 @@ def load(path: Optional[str] = None):
     lib.cp_sched_select_chunk.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                           C.c_int64, C.c_int32, C.c_int32, C.c_int32, C.c_int64,
                                           C.c_int32, C.POINTER(C.c_int32)]
+    lib.cp_decode_attention_static.argtypes = [C.c_void_p] * 4 + [C.c_int32] * 6 + [C.c_float, C.c_int32, C.c_void_p, C.c_void_p]
     if path is None:
         _lib = lib
     return lib
@@ -166,6 +168,17 @@ def _ptr(t) -> Optional[int]:
     if t is None:
         return None
     return int(t.data_ptr()) if hasattr(t, "data_ptr") else int(t)
+
+
+CP_STATIC_MAX_PARTIAL_ROWS = 4096
+
+
+def cp_decode_attention_static(q, kv_cache, block_tables, kv_len, n_reqs, max_pages_per_req, num_q_heads,
+                               num_kv_heads, head_dim, block_size, sm_scale, n_splits, out, stream=None):
+    """The no-allocation entry point (include/cp.h): device pointers / tensors in, two kernels enqueued, no context."""
+    _check(load().cp_decode_attention_static(_ptr(q), _ptr(kv_cache), _ptr(block_tables), _ptr(kv_len), n_reqs,
+                                             max_pages_per_req, num_q_heads, num_kv_heads, head_dim, block_size,
+                                             float(sm_scale), n_splits, _ptr(out), _ptr(stream)))
 
 
 class Context:

@@ -1,6 +1,7 @@
 """Build libcp.so in-tree for sm_100a (nvcc cross-compiles without a GPU).
 
   nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo   csrc/cp_api.cu   (kernels + C ABI)
+  nvcc (same flags)                                        csrc/cp_static.cu (the no-allocation entry point)
   g++  -ffp-contract=off                                   csrc/cp_sched.cpp (bit-exact fp64)
 The result, paper_2606_09061_b200/libcp.so, travels to the GPU box with the snapshot.
 """
@@ -43,6 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objs = []
     cmds = [
         ["nvcc", *nv, "-c", os.path.join(CSRC, "cp_api.cu"), "-o", os.path.join(OBJ, "cp_api.o")],
+        ["nvcc", *nv, "-c", os.path.join(CSRC, "cp_static.cu"), "-o", os.path.join(OBJ, "cp_static.o")],
         ["g++", *CXX_FLAGS, "-c", os.path.join(CSRC, "cp_sched.cpp"), "-o", os.path.join(OBJ, "cp_sched.o")],
         ["g++", *CXX_FLAGS, "-c", os.path.join(CSRC, "cp_error.cpp"), "-o", os.path.join(OBJ, "cp_error.o")],
     ]
