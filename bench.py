@@ -304,7 +304,7 @@ def run_ours(args):
     e2e_ms = e0.elapsed_time(e1)
     e2e_ms = max_over_ranks(e2e_ms, dev)
     ctx.cp_latency_table()
-    meta_bytes = 4 * (4 * spec.n_reqs + 2 + n_pages + spec.T) + 32 * (info.n_work_items + info.n_combine_items)
+    meta_bytes = 4 * (4 * spec.n_reqs + 2 + n_pages + spec.T) + 36 * info.n_work_items + 32 * info.n_combine_items
     h2d = int(hq.numel() * 2 + hk.numel() * 2 + hv_.numel() * 2 + meta_bytes)
     d2h = int(hout.numel() * 2)
 

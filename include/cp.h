@@ -212,10 +212,14 @@ int cp_set_memory_stats(cp_ctx* ctx, float gpu_mem_used_mb, float gpu_mem_free_m
 
 /* Introspection of the current batch (for tests and the roofline report). */
 typedef struct {
-    int32_t n_reqs, n_tokens, n_work_items, n_combine_items;
+    int32_t n_reqs, n_tokens, n_work_items;
+    int32_t n_combine_items;     /* split-KV groups of the batch: grid_combine of them are merged by the combine
+                                    kernel (chunk tiles), the others (decodes and <= 16-row chunk tails) inside the
+                                    attention kernel by the split that arrives last (no launch)                    */
     int32_t n_tc_items;          /* items routed to the tensor-core tile path      */
     int64_t n_partial_rows;      /* workspace rows in use                          */
-    int32_t kernels_per_step;    /* kernel launches one cp_attention_step issues   */
+    int32_t kernels_per_step;    /* kernel launches one cp_attention_step issues (append, attention; the combine
+                                    kernel only when grid_combine > 0; the scratch dequantisation for fp8 chunks) */
     int32_t grid_attn, grid_combine;
     double  alg_flops, alg_bytes; /* algorithmic work of ONE layer's step (SURVEY.md 8(d) formulas: FLOPs = 4 D Hq x causal
                                     pairs; bytes = KV once per request and KV head + Q + out + 4 B per page)          */

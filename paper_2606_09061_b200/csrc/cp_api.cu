@@ -74,6 +74,7 @@ struct cp_ctx {
     float* d_part_o = nullptr;
     float2* d_part_ml = nullptr;
     int32_t* d_counter = nullptr;      // persistent-kernel work counter
+    int32_t* d_group_cnt = nullptr;    // [max_combine] arrival counters of the groups merged inside the attention kernel (0 between launches)
     // rotary embedding fused into the append (cp_enable_rope); all null / -1 until enabled
     double* d_inv_freq = nullptr;      // [D/2]
     float2* d_rope_cs = nullptr;       // [max_tokens][D/2] (cos, sin) of the current batch's positions
@@ -107,8 +108,8 @@ struct cp_ctx {
 
     // host scratch reused across build_batch calls (no allocation in steady state)
     std::vector<WorkItem> items, sorted;
-    std::vector<CombineItem> combines;
-    std::vector<int32_t> bucket, plan, plan_prow;
+    std::vector<CombineItem> combines, fused;   // groups merged by combine_kernel / inside the attention kernel (swap kind)
+    std::vector<int32_t> bucket, plan, plan_prow, plan_aux, aux, sorted_aux;
 #ifdef CP_DEBUG_VARIANTS
     std::vector<uint32_t> page_mark;   // debug builds: page -> number of the last build that named it
     uint32_t mark_epoch = 0;
@@ -173,6 +174,7 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     c->max_scratch_pages = c->kv8 ? (cfg->max_scratch_pages > 0 ? cfg->max_scratch_pages : cfg->max_total_pages) : 0;
     if (c->kv8) cap += align_up(sizeof(int32_t) * cfg->max_reqs, 16) + align_up(sizeof(int32_t) * (size_t)c->max_scratch_pages, 16);
     cap += align_up(sizeof(WorkItem) * c->max_items, 16);
+    cap += align_up(sizeof(int32_t) * c->max_items, 16);                 // work_aux
     cap += align_up(sizeof(CombineItem) * c->max_combine, 16);
     c->meta_cap = cap;
 
@@ -182,6 +184,8 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     chk(cudaMalloc(&c->d_part_o, sizeof(float) * (size_t)c->max_partial_rows * D));
     chk(cudaMalloc(&c->d_part_ml, sizeof(float2) * (size_t)c->max_partial_rows));
     chk(cudaMalloc(&c->d_counter, sizeof(int32_t) * 4));
+    chk(cudaMalloc(&c->d_group_cnt, sizeof(int32_t) * c->max_combine));
+    if (e == cudaSuccess) chk(cudaMemset(c->d_group_cnt, 0, sizeof(int32_t) * c->max_combine));
     if (c->kv8) chk(cudaMalloc(&c->d_scratch, sizeof(__nv_bfloat16) * (size_t)c->max_scratch_pages * 2 * Hkv * cfg->block_size * D));
     chk(cudaMemset(c->d_counter, 0, sizeof(int32_t) * 4));
     for (int i = 0; i < kMetaRing; ++i) {
@@ -206,6 +210,10 @@ extern "C" int cp_create(const cp_config* cfg, cp_ctx** out) {
     c->items.reserve(c->max_items);
     c->sorted.reserve(c->max_items);
     c->combines.reserve(c->max_combine);
+    c->fused.reserve(c->max_combine);
+    c->plan_aux.reserve(q_tiles * Hkv);
+    c->aux.reserve(c->max_items);
+    c->sorted_aux.reserve(c->max_items);
     c->plan.reserve(2 * q_tiles);
     c->plan_prow.reserve(q_tiles * Hkv);
     *out = c;
@@ -220,6 +228,7 @@ extern "C" int cp_destroy(cp_ctx* c) {
     cudaFree(c->d_part_o);
     cudaFree(c->d_part_ml);
     cudaFree(c->d_counter);
+    cudaFree(c->d_group_cnt);
     cudaFree(c->d_scratch);
     cudaFree(c->d_inv_freq);
     cudaFree(c->d_rope_cs);
@@ -337,7 +346,9 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     int64_t partial_rows = 0;
     for (int attempt = 0;; ++attempt) {
         c->items.clear();
+        c->aux.clear();
         c->combines.clear();
+        c->fused.clear();
         partial_rows = 0;
         int64_t tok = 0;
         bool overflow = false;
@@ -347,6 +358,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
             const int nq = (r.q_len + TQ - 1) / TQ;
             c->plan.resize((size_t)nq * 2);                          // [qi] = {n_splits, tps}
             c->plan_prow.resize((size_t)nq * sh.Hkv);
+            c->plan_aux.resize((size_t)nq * sh.Hkv);
             int max_splits = 0;
             for (int qi = 0; qi < nq && !overflow; ++qi) {
                 const int q0 = qi * TQ, qt = std::min(TQ, r.q_len - q0), rows = qt * G;
@@ -357,16 +369,22 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
                 c->plan[2 * qi] = n_splits;
                 c->plan[2 * qi + 1] = (n_tiles + n_splits - 1) / n_splits;
                 max_splits = std::max(max_splits, n_splits);
+                // split groups of the swap kind are merged inside the attention kernel (the last split to arrive
+                // does it), the others by combine_kernel
+                const bool fuse = c->use_tc && rows <= swap_rows && sh.D == 128;
                 for (int g = 0; g < sh.Hkv; ++g) {
-                    int32_t prow = -1;
+                    int32_t prow = -1, aux = -1;
                     if (n_splits > 1) {
                         prow = (int32_t)partial_rows;
                         partial_rows += (int64_t)n_splits * rows;
                         if (partial_rows > c->max_partial_rows || partial_rows > INT32_MAX ||
-                            c->combines.size() >= c->max_combine) { overflow = true; break; }
-                        c->combines.push_back(CombineItem{(int32_t)(tok + q0), qt, g, n_splits, prow, 0, {0, 0}});
+                            c->combines.size() + c->fused.size() >= c->max_combine) { overflow = true; break; }
+                        const CombineItem ci{(int32_t)(tok + q0), qt, g, n_splits, prow, 0, {0, 0}};
+                        if (fuse) { aux = (int32_t)c->fused.size(); c->fused.push_back(ci); }
+                        else c->combines.push_back(ci);
                     }
                     c->plan_prow[(size_t)qi * sh.Hkv + g] = prow;
+                    c->plan_aux[(size_t)qi * sh.Hkv + g] = aux;
                 }
                 if (c->items.size() + (size_t)n_splits * sh.Hkv > c->max_items) overflow = true;
             }
@@ -385,6 +403,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
                         if (c->items.size() >= c->max_items) { overflow = true; break; }
                         c->items.push_back(WorkItem{j, g, q0, qt, s * tps * kKeyTile, std::min(lim, (s + 1) * tps * kKeyTile),
                                                     prow < 0 ? -1 : prow + s * rows, kind});
+                        c->aux.push_back(c->plan_aux[(size_t)qi * sh.Hkv + g]);
                         ++emitted;
                     }
             (void)emitted;
@@ -411,7 +430,12 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     for (const WorkItem& w : c->items) ++c->bucket[bucket_of(w) + 1];
     for (size_t i = 1; i < c->bucket.size(); ++i) c->bucket[i] += c->bucket[i - 1];
     c->sorted.resize(n_items);
-    for (const WorkItem& w : c->items) c->sorted[c->bucket[bucket_of(w)]++] = w;
+    c->sorted_aux.resize(n_items);
+    for (size_t i = 0; i < n_items; ++i) {
+        const size_t pos = c->bucket[bucket_of(c->items[i])]++;
+        c->sorted[pos] = c->items[i];
+        c->sorted_aux[pos] = c->aux[i];
+    }
 
     // ---- pack into pinned staging ------------------------------------------------------------
     // the batch that ends here: every step it will ever run has been enqueued on step_stream by now
@@ -430,7 +454,8 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     const size_t o_bt = place(sizeof(int32_t) * (size_t)P);
     const size_t o_tr = place(sizeof(int32_t) * (size_t)T);
     const size_t o_wk = place(sizeof(WorkItem) * n_items);
-    const size_t o_cb = place(sizeof(CombineItem) * c->combines.size());
+    const size_t o_wa = place(sizeof(int32_t) * n_items);
+    const size_t o_cb = place(sizeof(CombineItem) * (c->combines.size() + c->fused.size()));      // [combine_kernel's | fused]
     // fp8 pools: requests with a tile-kind item get their pages dequantised into the scratch pool, contiguously
     size_t o_sb = 0, o_sr = 0;
     if (c->kv8) {
@@ -474,12 +499,14 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
         for (int i = 0; i < r.q_len; ++i) tr[cu[j] + i] = j;
     }
     std::memcpy(h + o_wk, c->sorted.data(), sizeof(WorkItem) * n_items);
+    std::memcpy(h + o_wa, c->sorted_aux.data(), sizeof(int32_t) * n_items);
     {   // prefix sums of the groups' row counts: the combine kernel maps one warp to one row
         int32_t rows = 0;
         for (CombineItem& ci : c->combines) { ci.row_base = rows; rows += ci.q_tokens * G; }
         c->combine_rows = rows;
     }
     std::memcpy(h + o_cb, c->combines.data(), sizeof(CombineItem) * c->combines.size());
+    std::memcpy(h + o_cb + sizeof(CombineItem) * c->combines.size(), c->fused.data(), sizeof(CombineItem) * c->fused.size());
     if (c->kv8) {
         std::memcpy(h + o_sb, c->scratch_base.data(), sizeof(int32_t) * n_reqs);
         std::memcpy(h + o_sr, c->scratch_req.data(), sizeof(int32_t) * c->scratch_req.size());
@@ -505,6 +532,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
     m.block_table = reinterpret_cast<const int32_t*>(d_meta + o_bt);
     m.tok_req = reinterpret_cast<const int32_t*>(d_meta + o_tr);
     m.work = reinterpret_cast<const WorkItem*>(d_meta + o_wk);
+    m.work_aux = reinterpret_cast<const int32_t*>(d_meta + o_wa);
     m.combine = reinterpret_cast<const CombineItem*>(d_meta + o_cb);
     m.scratch_base = c->kv8 ? reinterpret_cast<const int32_t*>(d_meta + o_sb) : nullptr;
     m.scratch_req = c->kv8 ? reinterpret_cast<const int32_t*>(d_meta + o_sr) : nullptr;
@@ -516,7 +544,7 @@ extern "C" int cp_build_batch(cp_ctx* c, const cp_req_desc* reqs, int32_t n_reqs
 
     int32_t n_tc = 0;
     if (c->use_tc) n_tc = (int32_t)n_items;
-    c->info = cp_batch_info{n_reqs, (int32_t)T, (int32_t)n_items, (int32_t)c->combines.size(), n_tc,
+    c->info = cp_batch_info{n_reqs, (int32_t)T, (int32_t)n_items, (int32_t)(c->combines.size() + c->fused.size()), n_tc,
                             partial_rows, 0, 0, 0,
                             4.0 * sh.D * sh.Hq * alg_pairs,
                             2.0 * alg_keys * sh.Hkv * (c->kv8 ? sh.D + 4.0 : sh.D * 2.0) + 2.0 * (double)T * sh.Hq * sh.D * 2 + 4.0 * (double)P,
@@ -667,7 +695,7 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const 
     }
     if (m.n_work > 0) {
         const int grid = std::min(c->n_sm, m.n_work);
-        dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, kv_scale};
+        dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, kv_scale, c->d_group_cnt};
         if (kv_scale) {
             if constexpr (D == 128)
                 CP_CUDA(launch_pdl(dl::attn_dl_kernel<128, false, false, true>, dim3(grid), dim3(dl::kThreads), dl::Layout<128, false>::kTotal, stream, p, tmap_copy, *tmap8));

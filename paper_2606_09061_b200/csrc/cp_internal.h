@@ -52,9 +52,11 @@ struct BatchMeta {
     const WorkItem* work;        // [n_work] sorted by descending cost
     const CombineItem* combine;  // [n_combine]
     const int32_t* tok_req;      // [T] request of each token (for the append kernel)
+    const int32_t* work_aux;     // [n_work] split item of a group merged INSIDE the attention kernel: its index among
+                                 // those groups (combine[n_combine + aux]); -1 otherwise
     const int32_t* scratch_base; // fp8 pools: [n_reqs] first page of the request in the bf16 scratch pool, -1 = none
     const int32_t* scratch_req;  // fp8 pools: [scratch pages in use] request of each scratch page
-    int32_t n_reqs, n_tokens, n_work, n_combine;
+    int32_t n_reqs, n_tokens, n_work, n_combine;   // n_combine: groups merged by combine_kernel (combine[0, n_combine))
     int32_t n_tile;              // dual-lane kernel: work[0, n_tile) are tile-kind items, the rest swap-kind
 };
 

@@ -129,6 +129,9 @@ struct LaneState {              // one per lane, in the misc region
     uint64_t item_full[kItemRing];
     uint64_t item_empty[kItemRing];
     WorkItem items[kItemRing];  // published by the lane's producer; kind < 0 = no more work
+    int32_t aux[kItemRing];     // BatchMeta::work_aux of the item
+    int32_t cur_aux;            // aux word of the item the lane's softmax warpgroup is working on (kept out of registers)
+    int32_t last_split;         // swap kind: this item's split was the last of its group to arrive
     float cmax[2][4][16];       // swap kind: per-warp column maxima, double buffered
     float lsum[4][16];          // swap kind: per-warp column sums at the end of an item
     float qs[8];                // fp8 swap kind: per-row scale of the quantised Q^T
@@ -149,6 +152,7 @@ struct Params {
     float2* part_ml;
     int32_t* counters;          // [0] next tile item, [1] next swap item, [2] finished CTAs
     const float* kv_scale;      // fp8 pools: [block][K|V][kv head][slot] power-of-two row scales, else unused
+    int32_t* group_cnt;         // [fused groups] arrivals of the splits of a group merged in this kernel (all 0 between launches)
 };
 
 // element e of a half-tile row: MUFU or FMA-pipe exponential (e is a constant after unrolling)
@@ -231,11 +235,13 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
                 idx = __shfl_sync(0xffffffffu, idx, 0);
                 idx = idx < p.meta.n_work - p.meta.n_tile ? idx + p.meta.n_tile : -1;
             }
-            w = 0;                               // one int32 of the 32-byte WorkItem per lane 0..7
+            w = 0;                               // one int32 of the 32-byte WorkItem per lane 0..7, its aux word in lane 8
             if (idx >= 0 && lane < 8) w = reinterpret_cast<const int32_t*>(p.meta.work + idx)[lane];
+            if (idx >= 0 && lane == 8) w = p.meta.work_aux[idx];
             if (idx < 0 && lane == 7) w = -1;    // kind = -1: sentinel
             ptx::mbar_wait(&ls->item_empty[islot], ((item_cnt / kItemRing) & 1) ^ 1);
             if (lane < 8) reinterpret_cast<int32_t*>(&ls->items[islot])[lane] = w;
+            if (lane == 8) ls->aux[islot] = w;
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(&ls->item_full[islot]);
         } else {
@@ -973,6 +979,76 @@ __device__ __forceinline__ void softmax_split(const WorkItem& it, const Params& 
 // (0, 2^8] whatever the scale), and the row sum takes w / vs = p back.  Q rows are scaled to amax 448 per row
 // (qs[c], folded into the score).  One lg2 per thread and tile; nothing per element beyond the bf16 kind.
 // ------------------------------------------------------------------------------------------
+// ------------------------------------------------------------------------------------------
+// Split-KV groups of the swap kind are merged INSIDE this kernel (H5 without a launch: the combine kernel and its
+// dependency hop cost a decode-only round 6-12 us per layer): every split writes its partial rows,
+// fences, and arrives on the group's counter; the split that arrives last merges all of them.  The counter is back
+// at 0 when the kernel ends.  Rolled loops, inlined (a call would put a stack frame into the kernel): it runs once per
+// group, outside every hot loop.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int arrive_split(const Params& p, int aux) {
+    const int n = p.meta.combine[p.meta.n_combine + aux].n_splits;
+    if (atomicAdd(&p.group_cnt[aux], 1) != n - 1) return 0;
+    p.group_cnt[aux] = 0;                                // nobody else touches it in this launch
+    return 1;
+}
+// The 4 warps of the warpgroup take the group's rows round-robin; per row the lanes first hold one split each
+// ((m_s, l_s) -> m = max m_s, w_s = 2^(m_s - m), sum w_s l_s by shuffles), then four d each: O = sum w_s O_s with the
+// weights broadcast by shuffle, so the loads of a row are independent and issue back to back (combine_kernel's scheme).
+__device__ __forceinline__ void merge_swap_group(const CombineItem* group, const float2* part_ml, const float* part_o,
+                                                 __nv_bfloat16* out, int G, int Hq, int warp, int lane) {
+    const CombineItem ci = *group;
+    const int R = ci.q_tokens * G, gs = 31 - __clz(G);     // G is a power of two (cp_create)
+    __threadfence();                                     // the other splits' rows were fenced before their arrival
+#pragma unroll 1
+    for (int r = warp; r < R; r += 4) {
+        // 32-bit offsets from the row's base pointers (n_splits * R * 128 stays far below 2^31)
+        const float2* ml_r = part_ml + ((int64_t)ci.partial_row + r);
+        const float* o_r = part_o + ((int64_t)ci.partial_row + r) * 128 + lane * 4;
+        float M = -INFINITY;
+#pragma unroll 1
+        for (int s = lane; s < ci.n_splits; s += 32) M = fmaxf(M, __ldcg(ml_r + s * R).x);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+        float L = 0.f, acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 1
+        for (int s0 = 0; s0 < ci.n_splits; s0 += 32) {
+            float w = 0.f;
+            if (s0 + lane < ci.n_splits) {
+                const float2 ml = __ldcg(ml_r + (s0 + lane) * R);
+                w = (ml.x == -INFINITY) ? 0.f : exp2f(ml.x - M);      // empty split: weight 0
+                L = fmaf(w, ml.y, L);                                  // this lane's share; summed over the lanes below
+            }
+            const int ns = min(32, ci.n_splits - s0);
+#pragma unroll 4
+            for (int j = 0; j < ns; ++j) {
+                const float wj = __shfl_sync(0xffffffffu, w, j);
+                const float4 v = __ldcg(reinterpret_cast<const float4*>(o_r + (s0 + j) * R * 128));
+                acc[0] = fmaf(wj, v.x, acc[0]); acc[1] = fmaf(wj, v.y, acc[1]);
+                acc[2] = fmaf(wj, v.z, acc[2]); acc[3] = fmaf(wj, v.w, acc[3]);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
+        const int tok = ci.tok0 + (r >> gs), head = ci.kv_head * G + (r & (G - 1));
+        const float inv = 1.f / L;
+        uint2 o2;
+        o2.x = pack_bf16(acc[0] * inv, acc[1] * inv);
+        o2.y = pack_bf16(acc[2] * inv, acc[3] * inv);
+        *reinterpret_cast<uint2*>(out + ((int64_t)tok * Hq + head) * 128 + lane * 4) = o2;
+    }
+}
+__device__ __forceinline__ void finish_swap_item(const Params& p, LaneState* ls, int d, int bar_id) {
+    const int aux = ls->cur_aux;
+    if (aux >= 0) {                                      // uniform over the 128 threads
+        __threadfence();                                 // this split's partial rows, before its arrival
+        ptx::named_bar_sync(bar_id, 128);
+        if (d == 0) ls->last_split = arrive_split(p, aux);
+        ptx::named_bar_sync(bar_id, 128);
+        if (ls->last_split) merge_swap_group(p.meta.combine + p.meta.n_combine + aux, p.part_ml, p.part_o, p.out, p.sh.G, p.sh.Hq, d >> 5, d & 31);
+    }
+}
+
 __device__ __forceinline__ uint32_t e4m3_of(float x) {             // round to nearest even, saturating
     uint16_t r;
     asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(r) : "f"(0.f), "f"(x));
@@ -1324,6 +1400,8 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
         const uint32_t islot = item_cnt % kItemRing;
         ptx::mbar_wait(&ls->item_full[islot], (item_cnt / kItemRing) & 1);
         const WorkItem it = ls->items[islot];
+        // (SPLIT: both warpgroups follow this ring, only the first works on swap-kind items)
+        if ((threadIdx.x & 127) == 0 && (!SPLIT || ROLE == 0)) ls->cur_aux = ls->aux[islot];    // read back in finish_swap_item, barriers in between
         warp_arrive(&ls->item_empty[islot]);
         if (it.kind < 0) break;
         if constexpr (SPLIT) {
@@ -1344,6 +1422,7 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
                 if (R <= 4) softmax_swap<LANE, 4>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
                 else if (R <= 8) softmax_swap<LANE, 8>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
                 else softmax_swap<LANE, 16>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
+                if (it.partial_row >= 0) finish_swap_item(p, ls, row, 1 + LANE);       // H5 for the item's group, if it is the last split
             }
         } else {
             if constexpr (ROLE == 0 && !SPLIT) softmax_tile<D, POLY>(it, p, ls, tmem, gh_tile, row, lane_base);

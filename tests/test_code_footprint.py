@@ -4,7 +4,10 @@ built libcp.so with cuobjdump).
 DESIGN.md 7.0: seven warp roles of `dl::attn_dl_kernel` run different code at once against the SM's 32 KB
 L1.5 instruction cache; at 19,216 SASS instructions (a `producer` copy per lane, runtime divisions by the
 GQA group size in column-unrolled code) a mixed batch spent 27 % of its issue slots waiting for instruction
-fetch and ran 1.4x slower.  The kernel is 14,632 instructions now; this test fails if it grows back.
+fetch and ran 1.4x slower.  The kernel was 14,560 instructions after that fix; this test fails if it grows back.
+Round 2 added ~600 instructions per softmax role for the in-kernel merge of split decode groups: it
+runs once per group, outside every per-tile loop, and the A/B on configs[2] showed no change -- the budgets below
+leave room for exactly that and nothing else.
 """
 import re
 import shutil
@@ -15,9 +18,9 @@ import pytest
 from paper_2606_09061_b200 import build
 
 # instantiation (D, POLY, SPLIT, KV8) -> budget in SASS instructions
-BUDGET = {"ILi128ELb0ELb0ELb0E": 15500,      # dual lane, bf16 pages: the HBM-bound mixed batch (the bench workload)
+BUDGET = {"ILi128ELb0ELb0ELb0E": 15900,      # dual lane, bf16 pages: the HBM-bound mixed batch (the bench workload)
           "ILi128ELb1ELb1ELb0E": 11500,      # SPLIT: tensor-bound batches
-          "ILi128ELb0ELb0ELb1E": 11500,      # dual lane over fp8 (e4m3) pages
+          "ILi128ELb0ELb0ELb1E": 11900,      # dual lane over fp8 (e4m3) pages
           "ILi64ELb0ELb0ELb0E": 4200, "ILi64ELb1ELb1ELb0E": 5400}
 
 

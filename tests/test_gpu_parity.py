@@ -239,6 +239,50 @@ def test_stress_long_decodes_with_chunk_no_deadlock():
     ctx.close()
 
 
+def test_split_decode_groups_are_merged_inside_the_attention_kernel():
+    """H5 without a launch: the split-KV groups of decodes (swap-kind items) are merged by the split that arrives
+    last, inside the attention kernel; a decode-only batch is two launches (append, attention).  Three steps in a row
+    on one batch with different Q, then another batch on the same context: the groups' arrival counters re-arm
+    themselves, stale partial rows of an earlier step never reach a result (out starts as NaN every time)."""
+    import torch
+    rng = np.random.default_rng(5)
+    ctx_a = list(rng.integers(3000, 20000, size=6)) + [1, 17, 300, 129]
+    spec = wl.make_spec("fused", 32, 8, 128, 16, 6000, [1] * len(ctx_a), [c - 1 for c in ctx_a], seed=51)
+    dev = torch.device("cuda:0")
+    ctx = gu.make_ctx(spec)
+    tabs = spec.compact_tables()
+    q, k_new, v_new, pool, compact = wl.device_values(spec, dev)
+    cache = gu.to_bits(compact)
+    ora.kv_append(gu.to_bits(k_new), gu.to_bits(v_new), cache, spec.q_len, spec.ctx_off, tabs)
+    ctx.cp_build_batch(spec.q_len, spec.ctx_off, spec.block_tables)
+    info = ctx.cp_get_batch_info()
+    assert info.n_combine_items > 0
+    for step in range(3):
+        if step:
+            q = (torch.randn(q.shape, device=dev, dtype=torch.float32, generator=torch.Generator(device=dev).manual_seed(step)) * 1.5).bfloat16()
+        out = torch.full((spec.T, spec.Hq, spec.D), float("nan"), device=dev, dtype=torch.bfloat16)
+        ctx.cp_attention_step(0, q, k_new if step == 0 else None, v_new if step == 0 else None, pool, out)
+        torch.cuda.synchronize()
+        want = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale)
+        got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)
+        gu.assert_close(got, want, f"fused merge, step {step}")
+    info = ctx.cp_get_batch_info()
+    assert info.grid_combine == 0 and info.kernels_per_step == 2          # no combine launch
+    # another batch on the same context: fewer, differently split groups reuse the counters and the workspace
+    sub = [0, 3, 6, 8]
+    spec2 = wl.BatchSpec("fused2", spec.Hq, spec.Hkv, spec.D, spec.B, spec.num_blocks, spec.q_len[sub], spec.ctx_off[sub],
+                         [spec.block_tables[j] for j in sub], spec.seed)
+    q2 = q[sub].contiguous()
+    out2 = torch.full((len(sub), spec.Hq, spec.D), float("nan"), device=dev, dtype=torch.bfloat16)
+    ctx.cp_build_batch(spec2.q_len, spec2.ctx_off, spec2.block_tables)
+    ctx.cp_attention_step(0, q2, None, None, pool, out2)
+    torch.cuda.synchronize()
+    want_all = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale)
+    got2 = wl.bf16_bits_to_f64(gu.to_bits(out2)).reshape(len(sub), spec.Hq, spec.D)
+    gu.assert_close(got2, want_all[sub], "fused merge, second batch")
+    ctx.close()
+
+
 @pytest.mark.parametrize("seed", range(100, 112))
 def test_fuzz_shapes_against_oracle(seed):
     """Randomised shapes: every supported group size, both head dims, ragged chunks, contexts long enough
