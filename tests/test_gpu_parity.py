@@ -283,6 +283,38 @@ def test_split_decode_groups_are_merged_inside_the_attention_kernel():
     ctx.close()
 
 
+def test_few_long_decodes_fit_one_round_of_the_lanes():
+    """A decode-only round with few long requests (what the configs[4] trace runs most of the time): cp_build_batch
+    picks the split length by the number of ROUNDS the lanes need, not by the mean load alone, so the
+    work list has at most one item per lane (2 lanes x SMs) and at most as many as the mean-load rule would give;
+    every row against the oracle (the merge of the split groups runs inside the attention kernel)."""
+    import torch
+    spec = wl.config_small_decode(seed=3)
+    dev = torch.device("cuda:0")
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    ctx = gu.make_ctx(spec)
+    q, k_new, v_new, pool, compact = wl.device_values(spec, dev)
+    cache = gu.to_bits(compact)
+    tabs = spec.compact_tables()
+    ora.kv_append(gu.to_bits(k_new), gu.to_bits(v_new), cache, spec.q_len, spec.ctx_off, tabs)
+    ctx.cp_build_batch(spec.q_len, spec.ctx_off, spec.block_tables)
+    info = ctx.cp_get_batch_info()
+    tiles = [(int(c) + 1 + 127) // 128 for c in spec.ctx_off]
+    mean_load = -(-sum(tiles) * spec.Hkv // (2 * n_sm))
+    by_mean_load = sum(-(-t // mean_load) for t in tiles) * spec.Hkv
+    assert by_mean_load > 2 * n_sm                      # the case the rule exists for: slightly more items than lanes
+    assert info.n_work_items <= 2 * n_sm and info.n_work_items <= by_mean_load
+    assert info.n_combine_items > 0 and info.n_work_items >= n_sm
+    out = torch.full((spec.T, spec.Hq, spec.D), float("nan"), device=dev, dtype=torch.bfloat16)
+    ctx.cp_attention_step(0, q, k_new, v_new, pool, out)
+    torch.cuda.synchronize()
+    assert ctx.cp_get_batch_info().kernels_per_step == 2
+    want = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale)
+    got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)
+    gu.assert_close(got, want, "12 long decodes")
+    ctx.close()
+
+
 @pytest.mark.parametrize("seed", range(100, 112))
 def test_fuzz_shapes_against_oracle(seed):
     """Randomised shapes: every supported group size, both head dims, ragged chunks, contexts long enough
