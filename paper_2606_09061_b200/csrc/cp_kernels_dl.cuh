@@ -651,7 +651,7 @@ __device__ __forceinline__ void mma_warp(uint32_t smem_base, Misc* misc, int lan
 // tile), online softmax (log2 domain, lazy rescale), P row -> TMEM over the first 64 columns of the
 // same S buffer (bf16 pairs), O rescale / epilogue from TMEM.
 // ------------------------------------------------------------------------------------------
-template <int D, bool POLY>
+template <int D, bool POLY, bool NARROW>      // NARROW: 200 registers per thread (fp8 pools: one code copy for both softmax warpgroups)
 __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p, LaneState* ls, uint32_t tmem,
                                              uint32_t& gh, int row, uint32_t lane_base) {
     const Shape& sh = p.sh;
@@ -768,6 +768,32 @@ __device__ __forceinline__ void softmax_tile(const WorkItem& it, const Params& p
     ptx::mbar_wait(&ls->tpv_done[(gh - 1) & 3], ((gh - 1) >> 2) & 1);
     ptx::tc_fence_after();
     const float inv = 1.f / l;
+    if constexpr (NARROW) {
+#pragma unroll 1
+        for (int c = 0; c < D / 64; ++c) {               // 64 columns at a time
+            uint32_t o[64];
+            ptx::tmem_ld32(t_row + col_o(0) + c * 64, o);
+            ptx::tmem_ld32(t_row + col_o(0) + c * 64 + 32, o + 32);
+            ptx::tmem_wait_ld();
+            if (!valid_row) continue;
+            if (it.partial_row < 0) {
+                uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * sh.Hq + head) * D + c * 64);
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    dst[j] = make_uint4(pack_bf16(__uint_as_float(o[8 * j]) * inv, __uint_as_float(o[8 * j + 1]) * inv),
+                                        pack_bf16(__uint_as_float(o[8 * j + 2]) * inv, __uint_as_float(o[8 * j + 3]) * inv),
+                                        pack_bf16(__uint_as_float(o[8 * j + 4]) * inv, __uint_as_float(o[8 * j + 5]) * inv),
+                                        pack_bf16(__uint_as_float(o[8 * j + 6]) * inv, __uint_as_float(o[8 * j + 7]) * inv));
+            } else {
+                uint4* dst = reinterpret_cast<uint4*>(p.part_o + ((int64_t)it.partial_row + row) * D + c * 64);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) dst[j] = make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+            }
+        }
+        if (valid_row && it.partial_row >= 0) p.part_ml[(int64_t)it.partial_row + row] = make_float2(m_ref, l);
+        ptx::tc_fence_before();
+        return;
+    }
     uint32_t o[D];
 #pragma unroll
     for (int c = 0; c < D / 32; ++c) ptx::tmem_ld32(t_row + col_o(0) + c * 32, o + c * 32);
@@ -1060,9 +1086,9 @@ __device__ __forceinline__ float e4m3_value(uint32_t code) {
     return __half2float(__ushort_as_half((unsigned short)(h2 & 0xffffu)));
 }
 
-template <int LANE, int RC>
+template <int RC>
 __device__ __forceinline__ void softmax_swap8(const WorkItem& it, const Params& p, uint8_t* small, LaneState* ls,
-                                              uint32_t tmem, uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base, int swarp) {
+                                              uint32_t tmem, uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base, int swarp, int LANE) {
     constexpr int D = 128;
     const Shape& sh = p.sh;
     const int G = sh.G;
@@ -1249,9 +1275,9 @@ __device__ __forceinline__ void softmax_swap8(const WorkItem& it, const Params& 
     ptx::named_bar_sync(1 + LANE, 128);                  // lsum / cmax / qs are reused by the next item
 }
 // ------------------------------------------------------------------------------------------
-template <int LANE, int RC>
+template <int RC>
 __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p, uint8_t* small, LaneState* ls,
-                                             uint32_t tmem, uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base, int swarp) {
+                                             uint32_t tmem, uint32_t& gt, uint32_t& gp, int row, uint32_t lane_base, int swarp, int LANE) {
     constexpr int D = 128;
     const Shape& sh = p.sh;
     const int G = sh.G;
@@ -1386,15 +1412,19 @@ __device__ __forceinline__ void softmax_swap(const WorkItem& it, const Params& p
 // ROLE 2: lane S.
 // SPLIT: all warpgroups follow lane 0's item ring; ROLE 0 = warpgroup 0 of the column split (and the swap-kind
 // items), ROLE 2 = warpgroups wg >= 1 (swap-kind items are skipped).
-template <int D, int ROLE, bool POLY, bool SPLIT, bool KV8>
-__device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Misc* misc, int warp, int lane, int wg = 0) {
+template <int D, bool POLY, bool SPLIT, bool KV8>
+__device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Misc* misc, int warp, int lane, int ROLE, int wg) {
     using L = Layout<D, SPLIT>;
-    constexpr int LANE = (ROLE == 2 && !SPLIT) ? 1 : 0;
+    // ROLE is a warp-uniform runtime value (as the lane is in producer()): where the kernel calls this from ONE site
+    // (fp8 pages) one copy of the code serves both softmax warpgroups; where it calls it once per warpgroup with a
+    // constant, each call is specialised as if ROLE were a template parameter (bf16 pages)
+    const int LANE = (ROLE == 2 && !SPLIT) ? 1 : 0;
     LaneState* ls = &misc->lane[LANE];
     const uint32_t tmem = misc->tmem_base;
     const uint32_t lane_base = (warp & 3) * 32;
     const int row = lane_base + lane;
-    uint8_t* small = smem + L::kOffSmall[LANE];
+    constexpr uint32_t kOffSmall0 = L::kOffSmall[0], kOffSmall1 = L::kOffSmall[1];
+    uint8_t* small = smem + (LANE == 0 ? kOffSmall0 : kOffSmall1);
     uint32_t gt = 0, item_cnt = 0, gh_tile = 0, gp_swap = 0;      // gt / gp_swap: swap-kind tiles; gh_tile: tile-kind half-tiles
     for (;;) {
         const uint32_t islot = item_cnt % kItemRing;
@@ -1416,16 +1446,16 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
             if constexpr (D == 128) {
                 const int R = it.q_tokens * p.sh.G;
                 if constexpr (KV8) {
-                    if (R <= 4) softmax_swap8<LANE, 4>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
-                    else softmax_swap8<LANE, 8>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
+                    if (R <= 4) softmax_swap8<4>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3, LANE);
+                    else softmax_swap8<8>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3, LANE);
                 } else
-                if (R <= 4) softmax_swap<LANE, 4>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
-                else if (R <= 8) softmax_swap<LANE, 8>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
-                else softmax_swap<LANE, 16>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3);
+                if (R <= 4) softmax_swap<4>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3, LANE);
+                else if (R <= 8) softmax_swap<8>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3, LANE);
+                else softmax_swap<16>(it, p, small, ls, tmem, gt, gp_swap, row, lane_base, warp & 3, LANE);
                 if (it.partial_row >= 0) finish_swap_item(p, ls, row, 1 + LANE);       // H5 for the item's group, if it is the last split
             }
         } else {
-            if constexpr (ROLE == 0 && !SPLIT) softmax_tile<D, POLY>(it, p, ls, tmem, gh_tile, row, lane_base);
+            if constexpr (!SPLIT) softmax_tile<D, POLY, KV8>(it, p, ls, tmem, gh_tile, row, lane_base);
         }
         ++item_cnt;
     }
@@ -1498,12 +1528,20 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap, const _
         else if (SPLIT) { }                                                                      // SPLIT: warps 6, 7 have no role
         else if (warp == 6) mma_warp<D, 0, 2, false, KV8>(ptx::smem_u32(smem), misc, lane);     // lane T: PV blocks
         else mma_warp<D, 1, 0, false, KV8>(ptx::smem_u32(smem), misc, lane);                    // lane S
+    } else if (KV8) {
+        // fp8 pages: ONE call site, so both softmax warpgroups run the same code copy and take the same register
+        // budget (2 x 128 x 200 + 256 x 56 = 64 K registers).  A copy of the fp8 decode softmax per warpgroup did not
+        // fit the instruction cache (stall_no_instruction 2.2 per issue): 512 decodes 334 -> 296 us.
+        reg_inc<200>();
+        softmax_warps<D, POLY, SPLIT, KV8>(p, smem, misc, warp, lane, warp < 12 ? 0 : 2, 0);
     } else if (warp < 12) {
+        // bf16 pages: a copy per warpgroup, each with the register budget its role wants -- the shared copy measured
+        // 0.6 % slower on configs[2] (626 against 622 us) and 0.4-0.8 % slower in SPLIT mode (A/B on one box)
         reg_inc<kWide ? 96 : SPLIT ? 200 : 232>();
-        softmax_warps<D, 0, POLY, SPLIT, KV8>(p, smem, misc, warp, lane);
+        softmax_warps<D, POLY, SPLIT, KV8>(p, smem, misc, warp, lane, 0, 0);
     } else {
         reg_inc<kWide ? 96 : SPLIT ? 200 : 160>();
-        softmax_warps<D, 2, SPLIT && POLY, SPLIT, KV8>(p, smem, misc, warp, lane, (warp - 8) >> 2);
+        softmax_warps<D, POLY, SPLIT, KV8>(p, smem, misc, warp, lane, 2, (warp - 8) >> 2);
     }
     ptx::tc_fence_before();
     __syncthreads();

@@ -7,7 +7,8 @@ GQA group size in column-unrolled code) a mixed batch spent 27 % of its issue sl
 fetch and ran 1.4x slower.  The kernel was 14,560 instructions after that fix; this test fails if it grows back.
 Round 2 added ~600 instructions per softmax role for the in-kernel merge of split decode groups: it
 runs once per group, outside every per-tile loop, and the A/B on configs[2] showed no change -- the budgets below
-leave room for exactly that and nothing else.
+leave room for exactly that and nothing else.  The fp8 instantiation went from 11,760 to 7,928 instructions when its
+two softmax warpgroups began to share one code copy (512 decodes over fp8 pages 334 -> 296 us).
 """
 import re
 import shutil
@@ -20,7 +21,7 @@ from paper_2606_09061_b200 import build
 # instantiation (D, POLY, SPLIT, KV8) -> budget in SASS instructions
 BUDGET = {"ILi128ELb0ELb0ELb0E": 15900,      # dual lane, bf16 pages: the HBM-bound mixed batch (the bench workload)
           "ILi128ELb1ELb1ELb0E": 11500,      # SPLIT: tensor-bound batches
-          "ILi128ELb0ELb0ELb1E": 11900,      # dual lane over fp8 (e4m3) pages
+          "ILi128ELb0ELb0ELb1E": 8100,       # dual lane over fp8 (e4m3) pages: ONE softmax code copy for both warpgroups
           "ILi64ELb0ELb0ELb0E": 4200, "ILi64ELb1ELb1ELb0E": 5400}
 
 
