@@ -191,9 +191,11 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
 // producer warps of a lane.  Producer 0 fetches work items (atomic counters) and publishes them to
 // the lane's other warps through a small smem ring; all kProd producers stream the K and V tiles of
 // each item into the lane's slot ring in consumption order K0, K1, V0, K2, V1, ..., K(n-1), V(n-2),
-// V(n-1), load number ld (counted over the whole kernel) going to producer ld mod kProd.  A warp sustains one TMA box (one 4 KiB page slab)
-// per ~230 cycles, i.e. ~3700 cycles per 128-key K+V tile pair: one producer per lane caps a lane at
-// ~33 GB/s and was the bound of both lanes; the issue rate scales with the number of warps.
+// V(n-1), load number ld (counted over the whole kernel) going to producer ld mod kProd.  The eight boxes (4 KiB page
+// slabs) of a tile are issued by eight lanes of the warp in ONE instruction: a single thread sustains one box per
+// ~230 cycles, so a leader issuing them one after the other held a ring slot ~1800 cycles before its last byte was
+// even requested -- with three slots per lane that capped the decode lane of a mixed batch at ~39 GB/s (148 lanes:
+// 5.8 TB/s, below the HBM rate) while lane T was busy with chunk tiles (configs[2] 629 -> 608 us).
 // Together the producers run ahead of the consumers by up to kStages tile loads, across item
 // boundaries.  Page ids are prefetched 32 at a time (one per lane of the warp, two windows; each
 // producer's tile sequence is monotone) so no dependent global load sits between two TMA issues.
@@ -286,14 +288,17 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1);
             const bool leader = ptx::elect_one();
             if (leader) ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * (fp8_item ? kPage8Bytes : 16u * D * 2u));
+            __syncwarp();
             uint8_t* dst = kv_base + slot * slot_bytes;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
+            // lanes 0 .. n_pages-1 issue one box (page slab) each, in ONE warp instruction: a leader issuing the eight boxes
+            // of a tile one after the other held the slot ~1800 cycles before its last byte was even requested
+            {
+                const int j = lane & 7;
                 const int pg = __shfl_sync(0xffffffffu, cur, (tile & 3) * 8 + j);
-                if (j < n_pages) {
+                if (lane < n_pages) {
                     const int slab = (pg * 2 + is_v) * p.sh.Hkv + kv_head;
-                    if (KV8 && fp8_item) { if (leader) ptx::tma_load_3d(dst + j * kPage8Bytes, tmap8, &ls->kv_full[slot], 0, 0, slab); }
-                    else if (leader) ptx::tma_load_5d(dst + j * L::kPageBytes, tmap, &ls->kv_full[slot], 0, 0, 0, 0, slab);
+                    if (KV8 && fp8_item) ptx::tma_load_3d(dst + j * kPage8Bytes, tmap8, &ls->kv_full[slot], 0, 0, slab);
+                    else ptx::tma_load_5d(dst + j * L::kPageBytes, tmap, &ls->kv_full[slot], 0, 0, 0, 0, slab);
                 }
             }
             __syncwarp();
