@@ -816,8 +816,7 @@ static int issue_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new
             CP_CUDA(cudaGetLastError());
             ++launches;
             if (c->scratch_pages > 0) {
-                const int64_t units = (int64_t)c->scratch_pages * 2 * sh.Hkv * sh.B * (sh.D / 16);
-                const int g2 = (int)std::min<int64_t>((units + 255) / 256, (int64_t)c->n_sm * 16);
+                const int g2 = (int)std::min<int64_t>(c->scratch_pages, (int64_t)c->n_sm * 8);      // a CTA per scratch page
                 kv8_dequant_kernel<<<g2, 256, 0, stream>>>(m, sh, static_cast<const uint8_t*>(kv_cache), static_cast<const float*>(kv_scale),
                                                            c->d_scratch, c->scratch_pages);
                 CP_CUDA(cudaGetLastError());

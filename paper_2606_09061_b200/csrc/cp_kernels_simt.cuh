@@ -262,38 +262,45 @@ __global__ void kv_append_q8_kernel(BatchMeta meta, Shape sh, const uint4* __res
 
 // kv8_dequant_kernel: the pages of every request that has a prefill chunk -> the bf16 scratch pool, page p of
 // request j at scratch page scratch_base[j] + p, same slab layout as a bf16 pool.  code_value * 2^e is exact in
-// bf16 (4 significant bits), so the chunk tiles then compute on exactly the values the fp8 pages hold.  One
-// thread per 16-byte chunk of codes.  Unused slots of a last page were cleared by the append kernel (code 0).
-__global__ void kv8_dequant_kernel(BatchMeta meta, Shape sh, const uint8_t* __restrict__ cache8,
-                                   const float* __restrict__ scales, __nv_bfloat16* __restrict__ scratch,
-                                   int32_t n_scratch_pages) {
-    const int chunks = sh.D / 16;
-    const int64_t per_page = (int64_t)2 * sh.Hkv * sh.B * chunks;
-    const int64_t total = (int64_t)n_scratch_pages * per_page;
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
-         i += (int64_t)gridDim.x * blockDim.x) {
-        const int sp = (int)(i / per_page);                       // scratch page
-        const int64_t w = i % per_page;                           // (kv, head, slot, chunk) within the page
-        const int req = meta.scratch_req[sp];
-        const int64_t page = meta.block_table[meta.bt_off[req] + (sp - meta.scratch_base[req])];
-        const int64_t row_in_page = w / chunks;                   // (kv * Hkv + head) * B + slot
-        const int c = (int)(w % chunks);
-        const int64_t src_row = page * 2 * sh.Hkv * sh.B + row_in_page;
-        const uint4 codes = *reinterpret_cast<const uint4*>(cache8 + src_row * sh.D + c * 16);
-        const float sc = scales[src_row];
-        const uint16_t* c2 = reinterpret_cast<const uint16_t*>(&codes);
-        uint4 o[2];
-        __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(o);
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            uint32_t h2;
-            asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"(c2[j]));
-            const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h2));
-            ob[j] = __floats2bfloat162_rn(f.x * sc, f.y * sc);
+// bf16 (4 significant bits), so the chunk tiles then compute on exactly the values the fp8 pages hold.  One CTA
+// per scratch page (grid-stride): the page's id is looked up ONCE per CTA (the first version did the four dependent
+// index loads and two 64-bit divisions per 16-byte chunk: 72 us for the 324 MB of configs[2]; HBM time 50 us), then
+// one thread per 16-byte chunk of codes, consecutive threads on consecutive chunks.  Unused slots of a last page
+// were cleared by the append kernel (code 0).
+__global__ void __launch_bounds__(256)
+kv8_dequant_kernel(BatchMeta meta, Shape sh, const uint8_t* __restrict__ cache8,
+                   const float* __restrict__ scales, __nv_bfloat16* __restrict__ scratch,
+                   int32_t n_scratch_pages) {
+    const int chunks = sh.D / 16;                                 // 16-byte chunks of codes per row
+    const int per_page = 2 * sh.Hkv * sh.B * chunks;              // (kv, head, slot, chunk)
+    __shared__ int64_t page_s;
+    for (int sp = blockIdx.x; sp < n_scratch_pages; sp += gridDim.x) {
+        __syncthreads();                                          // page_s of the previous page has been read
+        if (threadIdx.x == 0) {
+            const int req = meta.scratch_req[sp];
+            page_s = meta.block_table[meta.bt_off[req] + (sp - meta.scratch_base[req])];
         }
-        uint4* dst = reinterpret_cast<uint4*>(scratch + ((int64_t)sp * 2 * sh.Hkv * sh.B + row_in_page) * sh.D + c * 16);
-        dst[0] = o[0];
-        dst[1] = o[1];
+        __syncthreads();
+        const int64_t src_row0 = page_s * 2 * sh.Hkv * sh.B;
+        const int64_t dst_row0 = (int64_t)sp * 2 * sh.Hkv * sh.B;
+        for (int w = threadIdx.x; w < per_page; w += blockDim.x) {
+            const int row_in_page = w / chunks, c = w % chunks;   // (kv * Hkv + head) * B + slot
+            const uint4 codes = *reinterpret_cast<const uint4*>(cache8 + (src_row0 + row_in_page) * sh.D + c * 16);
+            const float sc = scales[src_row0 + row_in_page];
+            const uint16_t* c2 = reinterpret_cast<const uint16_t*>(&codes);
+            uint4 o[2];
+            __nv_bfloat162* ob = reinterpret_cast<__nv_bfloat162*>(o);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                uint32_t h2;
+                asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"(c2[j]));
+                const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h2));
+                ob[j] = __floats2bfloat162_rn(f.x * sc, f.y * sc);
+            }
+            uint4* dst = reinterpret_cast<uint4*>(scratch + (dst_row0 + row_in_page) * sh.D + c * 16);
+            dst[0] = o[0];
+            dst[1] = o[1];
+        }
     }
 }
 
