@@ -219,7 +219,9 @@ typedef struct {
     int32_t n_tc_items;          /* items routed to the tensor-core tile path      */
     int64_t n_partial_rows;      /* workspace rows in use                          */
     int32_t kernels_per_step;    /* kernel launches one cp_attention_step issues (append, attention; the combine
-                                    kernel only when grid_combine > 0; the scratch dequantisation for fp8 chunks) */
+                                    kernel only when grid_combine > 0; the scratch dequantisation for fp8 chunks;
+                                    a small decode-only batch over bf16 pages is ONE launch: the attention kernel
+                                    appends the new rows and clears the page tails itself)                        */
     int32_t grid_attn, grid_combine;
     double  alg_flops, alg_bytes; /* algorithmic work of ONE layer's step (SURVEY.md 8(d) formulas: FLOPs = 4 D Hq x causal
                                     pairs; bytes = KV once per request and KV head + Q + out + 4 B per page)          */

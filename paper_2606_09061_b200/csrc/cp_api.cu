@@ -710,9 +710,10 @@ static int get_tmap(cp_ctx* c, void* kv_cache, const CUtensorMap** out, int kind
 }
 
 // kv_scale != nullptr: kv_cache is an e4m3 pool (D = 128), chunk tiles read the library's bf16 scratch pool
+// k_new_fused / v_new_fused / fused: H2 runs inside the attention kernel (decode-only batches over bf16 pages)
 template <int D>
 static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const float* kv_scale, __nv_bfloat16* out,
-                       cudaStream_t stream, int* launches) {
+                       cudaStream_t stream, int* launches, bool fused, const void* k_new_fused, const void* v_new_fused) {
     const BatchMeta& m = c->meta;
     const CUtensorMap* tmap = nullptr;
     const CUtensorMap* tmap8 = nullptr;
@@ -725,13 +726,16 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const 
     if (!c->tc_attr_set) {
         CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D, false>::kTotal));
         CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<D, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<D, true>::kTotal));
-        if constexpr (D == 128)
+        if constexpr (D == 128) {
             CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<128, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<128, false>::kTotal));
+            CP_CUDA(cudaFuncSetAttribute(dl::attn_dl_kernel<128, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dl::Layout<128, false>::kTotal));
+        }
         c->tc_attr_set = true;
     }
     if (m.n_work > 0) {
         const int grid = std::min(c->n_sm, m.n_work);
-        dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, kv_scale, c->d_group_cnt};
+        dl::Params p{m, c->shape, q, out, c->d_part_o, c->d_part_ml, c->d_counter, kv_scale, c->d_group_cnt,
+                     static_cast<const uint4*>(k_new_fused), static_cast<const uint4*>(v_new_fused), static_cast<__nv_bfloat16*>(kv_cache)};
         if (kv_scale) {
             if constexpr (D == 128)
                 CP_CUDA(launch_pdl(dl::attn_dl_kernel<128, false, false, true>, dim3(grid), dim3(dl::kThreads), dl::Layout<128, false>::kTotal, stream, p, tmap_copy, *tmap8));
@@ -739,7 +743,10 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const 
         // Two instantiations of the one kernel, chosen per batch by the SURVEY.md 8(d) roofline formulas: HBM-bound
         // batches run chunk tiles and decode streams side by side (dual lane); tensor-bound batches put both softmax
         // warpgroups on every chunk tile (SPLIT) and move a quarter of the exponentials to the FMA pipe.
-        if (c->tensor_bound)
+        if (fused) {
+            if constexpr (D == 128)
+                CP_CUDA(launch_pdl(dl::attn_dl_kernel<128, false, false, false, true>, dim3(grid), dim3(dl::kThreads), dl::Layout<128, false>::kTotal, stream, p, tmap_copy, *tmap8));
+        } else if (c->tensor_bound)
             CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, true, true, false>, dim3(grid), dim3(dl::kThreadsSplit), dl::Layout<D, true>::kTotal, stream, p, tmap_copy, *tmap8));
         else
             CP_CUDA(launch_pdl(dl::attn_dl_kernel<D, false, false, false>, dim3(grid), dim3(dl::kThreads), dl::Layout<D, false>::kTotal, stream, p, tmap_copy, *tmap8));
@@ -757,9 +764,9 @@ static int launch_tc_d(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const 
 }
 
 static int launch_tc(cp_ctx* c, const __nv_bfloat16* q, void* kv_cache, const float* kv_scale, __nv_bfloat16* out,
-                     cudaStream_t stream, int* launches) {
-    return c->shape.D == 128 ? launch_tc_d<128>(c, q, kv_cache, kv_scale, out, stream, launches)
-                             : launch_tc_d<64>(c, q, kv_cache, kv_scale, out, stream, launches);
+                     cudaStream_t stream, int* launches, bool fused = false, const void* k_new = nullptr, const void* v_new = nullptr) {
+    return c->shape.D == 128 ? launch_tc_d<128>(c, q, kv_cache, kv_scale, out, stream, launches, fused, k_new, v_new)
+                             : launch_tc_d<64>(c, q, kv_cache, kv_scale, out, stream, launches, false, nullptr, nullptr);
 }
 
 // validate the arguments of one layer's step and enqueue its kernels (no events, no latency row)
@@ -791,8 +798,18 @@ static int issue_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new
     c->step_stream = stream;
     const BatchMeta& m = c->meta;
     int launches = 0;
+    // A small decode-only batch over bf16 pages (no tile-kind item: every request is one swap-kind q tile) needs no
+    // append launch: the attention kernel's producers write the new rows and clear the page tails themselves (H2 inside
+    // H4).  One kernel per layer instead of two dependent ones -- what a decode round of the configs[4] trace pays per
+    // layer: 16-layer submissions, 14 decodes of the trace's context mix 55.8 -> 52.3 us per layer, 14 short decodes
+    // 22.8 -> 20.2, 12 long decodes 149.7 -> 147.4, 70 decodes 86.0 -> 85.5.  With thousands of items the producers'
+    // extra work per item costs more than the launch it saves (512 decodes: 491 -> 510 us), hence the item limit.
+    const bool fused = c->use_tc && !rope && !c->kv8 && c->shape.D == 128 && m.n_tile == 0 && m.n_work > 0 &&
+                       m.n_work <= 4 * c->n_sm && !c->tensor_bound;
     if (m.n_tokens > 0) {
-        if (rope) {
+        if (fused) {
+            // nothing to launch here
+        } else if (rope) {
             const Shape& sh = c->shape;
             const int64_t total = (int64_t)m.n_tokens * (sh.Hkv * (sh.D / 8) + (sh.Hkv + sh.Hq) * (sh.D / 16));
             const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 8);
@@ -848,7 +865,7 @@ static int issue_step(cp_ctx* c, int32_t layer, const void* q, const void* k_new
 #endif
         {
             rc = launch_tc(c, static_cast<const __nv_bfloat16*>(q), kv_cache, static_cast<const float*>(kv_scale),
-                           static_cast<__nv_bfloat16*>(out), stream, &launches);
+                           static_cast<__nv_bfloat16*>(out), stream, &launches, fused, k_new, v_new);
         }
         if (rc != CP_OK) return rc;
     }

@@ -153,6 +153,10 @@ struct Params {
     int32_t* counters;          // [0] next tile item, [1] next swap item, [2] finished CTAs
     const float* kv_scale;      // fp8 pools: [block][K|V][kv head][slot] power-of-two row scales, else unused
     int32_t* group_cnt;         // [fused groups] arrivals of the splits of a group merged in this kernel (all 0 between launches)
+    // APPEND instantiation (decode-only batches over bf16 pages: H2 inside this kernel, no append launch)
+    const uint4* k_new;         // [T, Hkv, D] rows of the step, or nullptr (the caller wrote the pages: only the page tails are cleared)
+    const uint4* v_new;
+    __nv_bfloat16* cache;       // the pool the descriptors point into
 };
 
 // element e of a half-tile row: MUFU or FMA-pipe exponential (e is a constant after unrolling)
@@ -208,7 +212,12 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
 // 128-key tile; lane S's ring is six such slots, lane T's slots keep their 32 KiB stride); tile-kind items read
 // the request's dequantised pages from the library's bf16 scratch pool (tmap), where they are contiguous from
 // scratch_base[req] -- no block table.
-template <int D, bool SPLIT, bool KV8>
+// APPEND (decode-only batches): the producer that is about to load the K (V) tile holding positions of the step's new
+// tokens first copies their k_new (v_new) rows into the page slots -- and clears the slots of the request's last page
+// past its last key, as kv_append_kernel does -- then orders those generic-proxy stores before its TMA reads.  Tiles
+// are page-aligned and the splits of a request partition its keys, so every new row is written by exactly one warp
+// of one CTA, and only that warp reads the page in this launch.
+template <int D, bool SPLIT, bool KV8, bool APPEND>
 __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tmap, const CUtensorMap* tmap8, uint8_t* smem, Misc* misc, int lane, int warp) {
     using L = Layout<D, SPLIT>;
     static_assert(kStagesT == kStagesS, "the shared producer code assumes one ring depth");
@@ -259,6 +268,39 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
         const int n_tiles = (kv_end - kv_begin + kKeyTile - 1) / kKeyTile;
         const int32_t* bt = p.meta.block_table + p.meta.bt_off[req] + (kv_begin >> 4);
         const int n_pages_item = (kv_end - kv_begin + 15) >> 4;
+        int np0 = 0, np1 = 0;                            // APPEND: positions [np0, np1) of the request's new tokens
+        if constexpr (APPEND) {
+            np0 = p.meta.ctx_off[req];
+            np1 = np0 + p.meta.q_len[req];
+            if (np1 > kv_begin && np0 < kv_end) {        // the item's key range holds new rows (its last tiles)
+                // H2 for the tiles THIS warp will load, now: the stores are on their way while the item's earlier tiles stream
+                const int tok_base = p.meta.cu_q[req];
+                const int32_t* bt_req = p.meta.block_table + p.meta.bt_off[req];
+                constexpr int kChunks = D / 8;           // 16-byte chunks per row
+                const int tA = (max(np0, kv_begin) - kv_begin) / kKeyTile, tB = (min(np1, kv_end) - 1 - kv_begin) / kKeyTile;
+                for (int tt = tA; tt <= tB; ++tt)
+                    for (int is_v = 0; is_v < 2; ++is_v) {
+                        const int i = is_v ? (tt == n_tiles - 1 ? 2 * n_tiles - 1 : 2 * tt + 2) : (tt == 0 ? 0 : 2 * tt - 1);
+                        if ((int)((ld_base + i) % kProd) != pw) continue;      // another producer of the lane loads that tile
+                        const int t_lo = kv_begin + tt * kKeyTile, t_hi = min(kv_end, t_lo + kKeyTile);
+                        const int a = max(np0, t_lo), b = min(np1, t_hi);
+                        const uint4* src = is_v ? p.v_new : p.k_new;
+                        if (src)
+                            for (int u = lane; u < (b - a) * kChunks; u += 32) {
+                                const int pos = a + u / kChunks, c = u % kChunks;
+                                const int64_t page = bt_req[pos >> 4];
+                                __nv_bfloat16* dst = p.cache + (((page * 2 + is_v) * p.sh.Hkv + kv_head) * 16 + (pos & 15)) * (int64_t)D + c * 8;
+                                *reinterpret_cast<uint4*>(dst) = src[((int64_t)(tok_base + pos - np0) * p.sh.Hkv + kv_head) * kChunks + c];
+                            }
+                        if (np1 - 1 >= t_lo && np1 - 1 < t_hi) {      // the request's last key is in this tile: the tail of its page
+                            const int first_free = ((np1 - 1) & 15) + 1;
+                            const int64_t page = bt_req[(np1 - 1) >> 4];
+                            uint4* dst = reinterpret_cast<uint4*>(p.cache + (((page * 2 + is_v) * p.sh.Hkv + kv_head) * 16 + first_free) * (int64_t)D);
+                            for (int u = lane; u < (16 - first_free) * kChunks; u += 32) dst[u] = make_uint4(0, 0, 0, 0);
+                        }
+                    }
+            }
+        }
         const bool fp8_item = KV8 && __shfl_sync(0xffffffffu, w, 7) == kKindSwap;
         const bool scratch = KV8 && !fp8_item;
         const int sbase = scratch ? p.meta.scratch_base[req] + (kv_begin >> 4) : 0;
@@ -286,6 +328,16 @@ __device__ __forceinline__ void producer(const Params& p, const CUtensorMap* tma
             const uint32_t ld = ld_base + i;
             const uint32_t slot = ld % kStages;
             ptx::mbar_wait(&ls->kv_empty[slot], ((ld / kStages) & 1) ^ 1);
+            if constexpr (APPEND) {
+                // this tile holds new rows (written by this warp when the item began): order those generic-proxy stores
+                // before the TMA reads of the same bytes -- cheap by now, the stores landed long ago
+                const int t_lo = kv_begin + tile * kKeyTile;
+                if (np1 > t_lo && np0 < min(kv_end, t_lo + kKeyTile)) {      // warp-uniform
+                    __threadfence();
+                    asm volatile("fence.proxy.async;" ::: "memory");
+                    __syncwarp();
+                }
+            }
             const bool leader = ptx::elect_one();
             if (leader) ptx::mbar_arrive_expect_tx(&ls->kv_full[slot], (uint32_t)n_pages * (fp8_item ? kPage8Bytes : 16u * D * 2u));
             __syncwarp();
@@ -1471,10 +1523,11 @@ __device__ __forceinline__ void softmax_warps(const Params& p, uint8_t* smem, Mi
 // ------------------------------------------------------------------------------------------
 // KV8 (fp8 pools, dual-lane only): tmap = the library's bf16 scratch pool (chunk tiles), tmap8 = the e4m3 pool (decode
 // streams); otherwise tmap = the bf16 pool and tmap8 is a copy of it, unused.
-template <int D, bool POLY, bool SPLIT, bool KV8>
+template <int D, bool POLY, bool SPLIT, bool KV8, bool APPEND = false>
 __global__ void __launch_bounds__(threads_of<SPLIT>(), 1)
 attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap8) {
     static_assert(!(KV8 && (SPLIT || D != 128)), "fp8 pools: dual-lane instantiation, D = 128");
+    static_assert(!(APPEND && (SPLIT || KV8 || D != 128)), "fused append: decode-only batches over bf16 pages, D = 128");
     using L = Layout<D, SPLIT>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -1528,7 +1581,7 @@ attn_dl_kernel(const Params p, const __grid_constant__ CUtensorMap tmap, const _
     constexpr bool kWide = SPLIT && kSplitWG == 4;       // 8 warps x 48 + 16 warps x 96 = 24 warps x 80
     if (warp < 8) {
         reg_dec<kWide ? 48 : 56>();
-        if (warp < kProdT + kProdS) producer<D, SPLIT, KV8>(p, &tmap, &tmap8, smem, misc, lane, warp);
+        if (warp < kProdT + kProdS) producer<D, SPLIT, KV8, APPEND>(p, &tmap, &tmap8, smem, misc, lane, warp);
         else if (warp == 5) mma_warp<D, 0, 1, SPLIT, KV8>(ptx::smem_u32(smem), misc, lane);     // lane T: score blocks (and swap items); SPLIT: the one issuer
         else if (SPLIT) { }                                                                      // SPLIT: warps 6, 7 have no role
         else if (warp == 6) mma_warp<D, 0, 2, false, KV8>(ptx::smem_u32(smem), misc, lane);     // lane T: PV blocks

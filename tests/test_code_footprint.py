@@ -18,11 +18,12 @@ import pytest
 
 from paper_2606_09061_b200 import build
 
-# instantiation (D, POLY, SPLIT, KV8) -> budget in SASS instructions
-BUDGET = {"ILi128ELb0ELb0ELb0E": 15900,      # dual lane, bf16 pages: the HBM-bound mixed batch (the bench workload)
-          "ILi128ELb1ELb1ELb0E": 11500,      # SPLIT: tensor-bound batches
-          "ILi128ELb0ELb0ELb1E": 8100,       # dual lane over fp8 (e4m3) pages: ONE softmax code copy for both warpgroups
-          "ILi64ELb0ELb0ELb0E": 4200, "ILi64ELb1ELb1ELb0E": 5400}
+# instantiation (D, POLY, SPLIT, KV8, APPEND) -> budget in SASS instructions
+BUDGET = {"ILi128ELb0ELb0ELb0ELb0E": 15900,      # dual lane, bf16 pages: the HBM-bound mixed batch (the bench workload)
+          "ILi128ELb0ELb0ELb0ELb1E": 14600,      # the same with H2 inside (small decode-only batches: no tile items run, its tile code is cold)
+          "ILi128ELb1ELb1ELb0ELb0E": 11500,      # SPLIT: tensor-bound batches
+          "ILi128ELb0ELb0ELb1ELb0E": 8100,       # dual lane over fp8 (e4m3) pages: ONE softmax code copy for both warpgroups
+          "ILi64ELb0ELb0ELb0ELb0E": 4200, "ILi64ELb1ELb1ELb0ELb0E": 5400}
 
 
 @pytest.mark.skipif(shutil.which("cuobjdump") is None, reason="cuobjdump not on PATH")
@@ -45,7 +46,7 @@ def test_dual_lane_kernel_sass_size_within_budget():
         for name, n in hits.items():
             assert 1000 < n <= limit, f"{name}: {n} SASS instructions > budget {limit} (DESIGN.md 7.0)"
     # a runtime integer division shows up as a reciprocal sequence starting with I2F.U32.RP
-    for body in sass.split("attn_dl_kernelILi128ELb0ELb0ELb0E")[1:]:
+    for body in sass.split("attn_dl_kernelILi128ELb0ELb0ELb0ELb0E")[1:]:
         assert body.split("Function :", 1)[0].count("I2F.U32.RP") <= 4, "runtime integer divisions crept back"
 
 
@@ -63,7 +64,7 @@ def test_attention_kernel_is_blackwell_native():
     kernels = {k: v for k, v in bodies.items() if "attn_dl_kernel" in k}
     assert len(kernels) >= 4
     for name, body in kernels.items():
-        if "ELb1EEEv" in name:
+        if "ELb1ELb0EEEv" in name:               # KV8
             assert body.count("UTCQMMA") > 0, f"{name}: no fp8 tcgen05.mma (UTCQMMA) in the SASS"
         for mnemonic in ("UTCHMMA", "LDTM", "STTM", "UTMALDG", "UTCBAR"):
             assert body.count(mnemonic) > 0, f"{name}: no {mnemonic} in the SASS"

@@ -267,7 +267,7 @@ def test_split_decode_groups_are_merged_inside_the_attention_kernel():
         got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)
         gu.assert_close(got, want, f"fused merge, step {step}")
     info = ctx.cp_get_batch_info()
-    assert info.grid_combine == 0 and info.kernels_per_step == 2          # no combine launch
+    assert info.grid_combine == 0 and info.kernels_per_step == 1          # no combine launch, no append launch (H2 inside the attention kernel)
     # another batch on the same context: fewer, differently split groups reuse the counters and the workspace
     sub = [0, 3, 6, 8]
     spec2 = wl.BatchSpec("fused2", spec.Hq, spec.Hkv, spec.D, spec.B, spec.num_blocks, spec.q_len[sub], spec.ctx_off[sub],
@@ -308,10 +308,12 @@ def test_few_long_decodes_fit_one_round_of_the_lanes():
     out = torch.full((spec.T, spec.Hq, spec.D), float("nan"), device=dev, dtype=torch.bfloat16)
     ctx.cp_attention_step(0, q, k_new, v_new, pool, out)
     torch.cuda.synchronize()
-    assert ctx.cp_get_batch_info().kernels_per_step == 2
+    assert ctx.cp_get_batch_info().kernels_per_step == 1          # decode-only: the append runs inside the attention kernel
     want = ora.attention(gu.to_bits(q), cache, spec.q_len, spec.ctx_off, tabs, spec.sm_scale)
     got = wl.bf16_bits_to_f64(gu.to_bits(out)).reshape(spec.T, spec.Hq, spec.D)
     gu.assert_close(got, want, "12 long decodes")
+    # H2 parity of the fused append: every appended row bit for bit, the tail of each last page zero, nothing else touched
+    gu.assert_pages(gu.to_bits(pool)[spec.touched_pages()], cache, gu.keys_per_page(spec), "fused append")
     ctx.close()
 
 
