@@ -317,6 +317,36 @@ def test_few_long_decodes_fit_one_round_of_the_lanes():
     ctx.close()
 
 
+@pytest.mark.parametrize("Hq,Hkv", [(8, 2), (4, 4), (16, 1)])
+def test_fused_append_of_small_decode_only_batches(Hq, Hkv):
+    """Small batches without a tile-kind item run ONE kernel: the attention kernel's producers append the step's rows and
+    clear the page tails (include/cp.h).  Requests of 1..4 tokens (as many as still make a swap-kind item) whose new rows
+    start a request, straddle page and tile boundaries, end exactly on them, and sit behind long split contexts; NaN in
+    every stale slot; outputs against the oracle on every row, pages bit for bit; then a second step with k_new = NULL
+    (the caller wrote the pages: only the tails are cleared)."""
+    import torch
+    G = Hq // Hkv
+    qmax = 16 // G                                           # tokens of a swap-kind q tile
+    ctx_off = [0, 13, 14, 15, 16, 125, 126, 127, 128, 255, 1023, 5000, 20001]
+    q_len = [min(qmax, 1 + (i % 4)) for i in range(len(ctx_off))]
+    pages = sum((q + o + 15) // 16 for q, o in zip(q_len, ctx_off)) + 9
+    spec = wl.make_spec("fused_append", Hq, Hkv, 128, 16, pages, q_len, ctx_off, seed=77)
+    hv = wl.host_values(spec, poison=wl.NAN_BF16)
+    ctx = gu.make_ctx(spec)
+    got, pool_after = gu.run_gpu_host_values(spec, hv, 0, ctx=ctx, poison=wl.NAN_BF16)
+    info = ctx.cp_get_batch_info()
+    assert info.kernels_per_step == 1 and info.n_combine_items > 0
+    want, _ = gu.run_oracle_host_values(spec, wl.host_values(spec))
+    gu.assert_close(got, want, "fused append")
+    _, cache_nan = gu.run_oracle_host_values(spec, hv)
+    gu.assert_pages(pool_after[spec.touched_pages()], cache_nan, gu.keys_per_page(spec), "fused append")
+    got2, pool_after2 = gu.run_gpu_host_values(spec, hv, 0, append=False, ctx=ctx, poison=wl.NAN_BF16)
+    assert ctx.cp_get_batch_info().kernels_per_step == 1
+    gu.assert_close(got2, want, "fused tail clearing, caller-written pages")
+    gu.assert_pages(pool_after2[spec.touched_pages()], cache_nan, gu.keys_per_page(spec), "fused tail clearing")
+    ctx.close()
+
+
 @pytest.mark.parametrize("seed", range(100, 112))
 def test_fuzz_shapes_against_oracle(seed):
     """Randomised shapes: every supported group size, both head dims, ragged chunks, contexts long enough
